@@ -1,0 +1,142 @@
+/* dg.h -- C-ABI of the B200-native modal DG hot path of arXiv:2208.11131.
+ *
+ * One handle = one uniform periodic Cartesian mesh with tensor-product Legendre modes per cell
+ * (Eq. 6, 121-139 Eq. 13-16; mode set per DESIGN.md reading A1).  The hot path behind
+ * dg_step() is the per-Runge-Kutta-stage right-hand side of PAPER.md:175-190 (Eq. 20-21): modal -> Gauss
+ * points, volume flux integral (Euler flux Eq. 4, Navier-Stokes flux Eq. 37-39, artificial viscosity
+ * Eq. 24, 43-46), face reconstruction + HLLC + recovery-based viscous face flux
+ * (Eq. 27-36), lifting, the SSP-RK stage combine and the global CFL
+ * reduction (Eq. 23).  Every step runs in hand-written CUDA kernels for sm_100a; there is
+ * no CPU fallback: every entry point returns DG_ECUDA when no CUDA device / kernel image is usable.
+ *
+ * Conventions
+ *  - All functions return 0 (DG_OK) or a negative error code; nothing throws or aborts across the ABI.
+ *    dg_last_error() returns a static thread-local text for the last failing call.
+ *  - Pointers named `w`, `alpha`, `totals`, `out` may be HOST or DEVICE pointers (detected with
+ *    cudaPointerGetAttributes); they are caller-owned and only accessed during the call.  All device
+ *    state is library-owned and released by dg_free().
+ *  - State layout (external == internal for the conserved variables):
+ *        w[(mode*Vc + var)*Ncells + cell],  Vc = dim+2,
+ *        cell = (iz*Ny + iy)*Nx + ix,  mode = (lz*m + ly)*m + lx,  m = order,
+ *        var  = rho, rho v_x, rho v_y, (rho v_z), e      (Eq. 1-3).
+ *    The artificial-viscosity field alpha is one more modal field, layout
+ *        alpha[mode*Ncells + cell].
+ *  - `order` is the paper's p = n+1: n = highest Legendre degree per axis, m = n+1
+ *    Gauss points per axis.  1 <= order <= 8.
+ */
+#ifndef DG_B200_H
+#define DG_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define DG_OK            0
+#define DG_EINVAL       -1   /* bad mesh / order / count / option / null pointer */
+#define DG_ENOMEM       -2   /* device allocation failed */
+#define DG_EUNPHYSICAL  -3   /* rho <= 0 or p <= 0 met at an evaluation point during dg_step */
+#define DG_ECUDA        -4   /* CUDA runtime error, no device, or no sm_100a kernel image */
+
+typedef struct dg_solver dg_solver;   /* opaque, library-owned */
+
+/* Uniform Cartesian mesh of cubes (equal fixed cells of edge h). */
+typedef struct dg_mesh {
+    int    dim;          /* 2 or 3 */
+    int    ncell[3];     /* cells per axis x, y, z (ncell[2] ignored for dim = 2) */
+    double origin[3];    /* lower corner (informational: the operator is translation invariant) */
+    double h;            /* cell edge */
+    int    periodic[3];  /* must be 1 on every used axis (the five workloads are periodic) */
+} dg_mesh;
+
+/* Runtime options; defaults are the paper's. */
+typedef struct dg_options {
+    double f_cfl;        /* Courant factor of Eq. 23; default 0.5 */
+    int    rk_stages;    /* 1, 2 or 3: SSP-RK in Shu-Osher form; default 3 */
+    int    av_enable;    /* 1: carry the artificial-viscosity field alpha; default 0 */
+    double f_v;          /* shock source factor, Eq. 43; default 2.5 */
+    double f_tau;        /* decay time factor, Eq. 44; default 0.5 */
+    double f_w;          /* wiggle source factor, Eq. 45; default 0.2 */
+    double s_onset0;     /* S_onset = s_onset0 / order^2; default 1e-4 */
+    double alpha_max;    /* clamp of the point-wise alpha used in Eq. 46; default 1 */
+    double fixed_dt;     /* > 0: use this dt instead of Eq. 23; default 0 */
+    int    use_graph;    /* 1: replay each time step as a CUDA graph (default); 0: plain launches */
+} dg_options;
+
+/* Fill *opt with the defaults above. */
+int dg_default_options(dg_options *opt);
+
+/* Create a solver (PAPER.md:175-190 operator on `mesh`; gamma of Eq. 5; nu, chi of Eq. 37-39; nu = chi = 0
+ * selects the Euler path).  Allocates all device state; the state is zero until dg_set_state.
+ * opt may be NULL (defaults).  Errors: DG_EINVAL, DG_ENOMEM, DG_ECUDA. */
+int dg_init(dg_solver **out, const dg_mesh *mesh, int order, double gamma, double nu, double chi,
+            const dg_options *opt);
+
+/* Same as dg_init, but all device state lives in a caller-provided device buffer (e.g. a torch tensor):
+ * dg_workspace_bytes() gives the size needed; `device_workspace` must be 256-byte aligned, stay alive
+ * until dg_free() and is never freed by the library. */
+int dg_workspace_bytes(const dg_mesh *mesh, int order, const dg_options *opt, size_t *bytes);
+int dg_init_workspace(dg_solver **out, const dg_mesh *mesh, int order, double gamma, double nu, double chi,
+                      const dg_options *opt, void *device_workspace, size_t bytes);
+
+/* Run all later work of this solver on `cuda_stream` (a cudaStream_t passed as void*; NULL = default
+ * stream).  The Python binding passes torch's current stream. */
+int dg_set_stream(dg_solver *s, void *cuda_stream);
+
+/* Upload the modal state (layout above).  count must equal Vc*M*Ncells.  Resets alpha := 0, the sensor
+ * scalars := 0 and t := 0, and evaluates the wave speeds of Eq. 23 for the first step. */
+int dg_set_state(dg_solver *s, const double *w, size_t count);
+
+/* Overwrite the alpha field (count = M*Ncells); only valid with av_enable. */
+int dg_set_alpha(dg_solver *s, const double *alpha, size_t count);
+
+/* Advance nsteps full SSP-RK steps, each with its own Eq.-23 timestep (or fixed_dt).  All stages run on
+ * the device without host synchronisation; the call returns after the last step has finished.
+ * Returns DG_EUNPHYSICAL if any evaluation point saw rho <= 0 or p <= 0 (state then unspecified). */
+int dg_step(dg_solver *s, int nsteps);
+
+/* As dg_step but without the final synchronisation / flag read (for back-to-back timing);
+ * errors surface at the next dg_step / dg_sync / dg_get_state. */
+int dg_step_async(dg_solver *s, int nsteps);
+
+/* Wait for all queued work; returns DG_EUNPHYSICAL if the device flag is set. */
+int dg_sync(dg_solver *s);
+
+/* Download the modal state / alpha field. */
+int dg_get_state(dg_solver *s, double *w, size_t count);
+int dg_get_alpha(dg_solver *s, double *alpha, size_t count);
+
+/* |K| * sum_cells w_0 per conserved variable (mode 0 is the cell mean):
+ * totals[0] = mass, totals[1..dim] = momentum, totals[dim+1] = energy; unused entries are 0.
+ * `totals` is a HOST pointer to 5 doubles.  Deterministic fixed-shape reduction. */
+int dg_conserved_totals(dg_solver *s, double totals[5]);
+
+/* Evaluate dw/dt = L(w) (Eq. 20) of the current state without advancing it, for term-wise parity tests:
+ * out has the layout of the state (count = Vc*M*Ncells); alpha_out (may be NULL) that of alpha. */
+int dg_eval_rhs(dg_solver *s, double *out, size_t count, double *alpha_out, size_t alpha_count);
+
+/* Simulation time and the last timestep used (host pointers, either may be NULL). */
+int dg_get_time(dg_solver *s, double *t, double *last_dt);
+
+/* Launch geometry of the stage kernel of this solver (for bench.py / DESIGN.md): cells per block, threads
+ * per block, dynamic shared memory bytes per block, number of blocks.  Any pointer may be NULL. */
+int dg_kernel_info(dg_solver *s, int *cells_per_block, int *threads, int *smem_bytes, int *blocks);
+
+/* Number of kernel launches issued by this solver since dg_init (graph replays count their nodes). */
+int dg_launch_count(dg_solver *s, long long *count);
+
+/* Sustained fp64 FMA throughput of the device in FLOP/s, measured with a register-resident DFMA loop of
+ * `iters` iterations on every SM (roofline denominator for the ALU-bound configs). */
+int dg_measure_fp64_peak(int iters, double *flops_per_s, void *cuda_stream);
+
+/* Free all device state.  NULL is allowed. */
+int dg_free(dg_solver *s);
+
+/* Text of the last error on this thread ("" if none). */
+const char *dg_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DG_B200_H */

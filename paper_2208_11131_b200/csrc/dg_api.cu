@@ -1,0 +1,595 @@
+// C-ABI of the B200 DG solver (include/dg.h): handle, device state, time-step driver, small helper kernels.
+// The stage kernel itself lives in dg_stage.cuh and is instantiated per (dim, m) in dg_stage_inst.cu.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "../../include/dg.h"
+#include "dg_dispatch.h"
+#include "dg_tables.h"
+
+#include "dg_stage_args.h"
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+int fail(int code, const char *fmt, const char *detail = "") {
+    std::snprintf(g_err, sizeof(g_err), fmt, detail);
+    return code;
+}
+
+#define CU(call)                                                                     \
+    do {                                                                             \
+        cudaError_t e_ = (call);                                                     \
+        if (e_ != cudaSuccess) return fail(DG_ECUDA, #call ": %s", cudaGetErrorString(e_)); \
+    } while (0)
+
+typedef cudaError_t (*launch_fn)(int, int, const DgStageArgs *, cudaStream_t, int);
+typedef cudaError_t (*upload_fn)(const DgTables *);
+typedef void (*info_fn)(int, int, int *, int *, int *);
+typedef cudaError_t (*config_fn)(int, int);
+
+struct Dispatch {
+    launch_fn launch;
+    upload_fn upload;
+    info_fn info;
+    config_fn config;
+};
+
+#define DG_ENTRY(d, m) {DG_FN(dg_launch, d, m), DG_FN(dg_upload, d, m), DG_FN(dg_info, d, m), DG_FN(dg_config, d, m)},
+const Dispatch kDispatch[2][8] = {{DG_FOR_ALL_M(DG_ENTRY, 2)}, {DG_FOR_ALL_M(DG_ENTRY, 3)}};
+
+// ---- helper kernels -------------------------------------------------------------------------------
+
+// Eq. 23: dt = f_CFL h / (2 (n+1) (c_s,max + v_max)); advances t; re-arms the maxima.
+__global__ void dg_dt_kernel(double *scal, unsigned long long *maxbits, double f_cfl, double h, int order,
+                             double fixed_dt) {
+    const double cmax = __longlong_as_double((long long)maxbits[0]);
+    const double vmax = __longlong_as_double((long long)maxbits[1]);
+    const double dt = (fixed_dt > 0.0) ? fixed_dt : f_cfl * h / (2.0 * order * (cmax + vmax));
+    scal[0] = dt;
+    scal[1] += dt;
+    scal[2] = cmax;
+    scal[3] = vmax;
+    maxbits[0] = 0ull;
+    maxbits[1] = 0ull;
+}
+
+// |K| sum_cells w_0 per conserved variable: one block per variable, fixed-shape compensated reduction.
+__global__ void __launch_bounds__(1024) dg_totals_kernel(const double *w, int V, int ncells, double vol, double *out) {
+    __shared__ double ss[1024], sc[1024];
+    const int v = blockIdx.x;
+    const double *row = w + (size_t)v * ncells;   // mode 0, variable v
+    double s = 0.0, c = 0.0;                      // Neumaier summation
+    for (int i = threadIdx.x; i < ncells; i += 1024) {
+        const double x = row[i];
+        const double t = s + x;
+        c += (fabs(s) >= fabs(x)) ? ((s - t) + x) : ((x - t) + s);
+        s = t;
+    }
+    ss[threadIdx.x] = s;
+    sc[threadIdx.x] = c;
+    __syncthreads();
+    for (int o = 512; o > 0; o >>= 1) {
+        if (threadIdx.x < o) {
+            const double a = ss[threadIdx.x], b = ss[threadIdx.x + o];
+            const double t = a + b;
+            const double e = (fabs(a) >= fabs(b)) ? ((a - t) + b) : ((b - t) + a);
+            ss[threadIdx.x] = t;
+            sc[threadIdx.x] += sc[threadIdx.x + o] + e;
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) out[v] = vol * (ss[0] + sc[0]);
+}
+
+// register-resident DFMA loop: 8 independent chains per thread
+__global__ void __launch_bounds__(256) dg_dfma_kernel(double *out, int iters, double a, double b) {
+    double x0 = threadIdx.x, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+            x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+        }
+    }
+    const double s = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+    if (s == 12345.678) out[0] = s;   // never true for a = 1, b = 0 inputs; keeps the chains alive
+}
+
+}  // namespace
+
+struct dg_solver {
+    int dim, order, ncell[3], ncells;
+    double h, gamma, nu, chi;
+    dg_options opt;
+    int visc, av, Vc, V, M;
+    size_t nstate;          // V * M * ncells doubles
+    Dispatch fn;
+    cudaStream_t stream;
+    double *W0, *WA, *WB;
+    double *scal;           // [0] dt, [1] t, [2] cmax, [3] vmax, [8..12] totals
+    unsigned long long *maxbits;
+    int *flag;
+    double *sens_prev, *sens_new;
+    void *owned;            // cudaMalloc'ed block (NULL when the caller supplied the workspace)
+    bool speeds_valid;
+    cudaGraphExec_t graph;
+    long long launches;
+    int kC, kNT, kSmem;
+};
+
+namespace {
+
+size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+size_t workspace_layout(dg_solver *s, char *base) {
+    size_t off = 0;
+    auto take = [&](size_t bytes) {
+        char *p = base ? base + off : nullptr;
+        off += align_up(bytes, 256);
+        return p;
+    };
+    const size_t sb = s->nstate * sizeof(double);
+    s->W0 = (double *)take(sb);
+    s->WA = (double *)take(sb);
+    s->WB = (s->opt.rk_stages >= 3) ? (double *)take(sb) : nullptr;
+    s->scal = (double *)take(16 * sizeof(double));
+    s->maxbits = (unsigned long long *)take(2 * sizeof(unsigned long long));
+    s->flag = (int *)take(sizeof(int));
+    if (s->av) {
+        s->sens_prev = (double *)take(2 * (size_t)s->ncells * sizeof(double));
+        s->sens_new = (double *)take(2 * (size_t)s->ncells * sizeof(double));
+    } else {
+        s->sens_prev = s->sens_new = nullptr;
+    }
+    return off;
+}
+
+int validate(const dg_mesh *mesh, int order, double gamma, double nu, double chi, const dg_options *o) {
+    if (!mesh) return fail(DG_EINVAL, "mesh is NULL");
+    if (mesh->dim != 2 && mesh->dim != 3) return fail(DG_EINVAL, "mesh.dim must be 2 or 3");
+    if (order < 1 || order > DG_MAXM) return fail(DG_EINVAL, "order must be in 1..8");
+    double n = 1.0;
+    for (int a = 0; a < mesh->dim; ++a) {
+        if (mesh->ncell[a] < 1) return fail(DG_EINVAL, "mesh.ncell must be >= 1 on every used axis");
+        if (!mesh->periodic[a]) return fail(DG_EINVAL, "only periodic axes are supported");
+        n *= mesh->ncell[a];
+    }
+    if (n > 2.0e9) return fail(DG_EINVAL, "too many cells");
+    if (!(mesh->h > 0.0) || !std::isfinite(mesh->h)) return fail(DG_EINVAL, "mesh.h must be positive");
+    if (!(gamma > 1.0)) return fail(DG_EINVAL, "gamma must exceed 1");
+    if (!(nu >= 0.0) || !(chi >= 0.0)) return fail(DG_EINVAL, "nu and chi must be non-negative");
+    if (o->rk_stages < 1 || o->rk_stages > 3) return fail(DG_EINVAL, "rk_stages must be 1, 2 or 3");
+    if (!(o->f_cfl > 0.0) && !(o->fixed_dt > 0.0)) return fail(DG_EINVAL, "f_cfl must be positive");
+    return DG_OK;
+}
+
+void fill_args(const dg_solver *s, DgStageArgs *a) {
+    std::memset(a, 0, sizeof(*a));
+    a->scal = s->scal;
+    a->maxbits = s->maxbits;
+    a->flag = s->flag;
+    a->sens_prev = s->sens_prev;
+    a->sens_new = s->sens_new;
+    a->ncells = s->ncells;
+    a->nx = s->ncell[0];
+    a->ny = s->ncell[1];
+    a->nz = (s->dim == 3) ? s->ncell[2] : 1;
+    a->h = s->h;
+    a->gamma = s->gamma;
+    a->nu = s->nu;
+    a->chi = s->chi;
+    a->f_v = s->opt.f_v;
+    a->f_tau = s->opt.f_tau;
+    a->f_w = s->opt.f_w;
+    a->s_onset = s->opt.s_onset0 / ((double)s->order * (double)s->order);
+    a->alpha_max = s->opt.alpha_max;
+}
+
+// enqueue the wave-speed evaluation of the current state (Eq. 23 inputs for the next step)
+int enqueue_wavespeed(dg_solver *s) {
+    CU(cudaMemsetAsync(s->maxbits, 0, 2 * sizeof(unsigned long long), s->stream));
+    DgStageArgs a;
+    fill_args(s, &a);
+    a.w_prev = s->W0;
+    CU(s->fn.launch(s->visc, s->av, &a, s->stream, 1));
+    s->launches += 1;
+    s->speeds_valid = true;
+    return DG_OK;
+}
+
+// enqueue one full SSP-RK step (Shu-Osher forms)
+int enqueue_step(dg_solver *s) {
+    static const double A0[3][3] = {{1.0, 0, 0}, {1.0, 0.5, 0}, {1.0, 0.75, 1.0 / 3.0}};
+    static const double B1[3][3] = {{0.0, 0, 0}, {0.0, 0.5, 0}, {0.0, 0.25, 2.0 / 3.0}};
+    static const double CC[3][3] = {{1.0, 0, 0}, {1.0, 0.5, 0}, {1.0, 0.25, 2.0 / 3.0}};
+    const int S = s->opt.rk_stages;
+    dg_dt_kernel<<<1, 1, 0, s->stream>>>(s->scal, s->maxbits, s->opt.f_cfl, s->h, s->order, s->opt.fixed_dt);
+    CU(cudaGetLastError());
+    double *buf[2] = {s->WA, s->WB};
+    const double *prev = s->W0;
+    for (int i = 0; i < S; ++i) {
+        DgStageArgs a;
+        fill_args(s, &a);
+        double *out = (i == S - 1 && S > 1) ? s->W0 : buf[i % 2];
+        a.w_prev = prev;
+        a.w_n = s->W0;
+        a.w_out = out;
+        a.rk_a = A0[S - 1][i];
+        a.rk_b = B1[S - 1][i];
+        a.rk_c = CC[S - 1][i];
+        a.do_sensor = (i == 0) && s->av;
+        a.commit_sensor = (i == S - 1) && s->av;
+        a.do_wavespeed = (i == S - 1);
+        CU(s->fn.launch(s->visc, s->av, &a, s->stream, 0));
+        prev = out;
+    }
+    if (S == 1) CU(cudaMemcpyAsync(s->W0, s->WA, s->nstate * sizeof(double), cudaMemcpyDeviceToDevice, s->stream));
+    return DG_OK;
+}
+
+int check_flag(dg_solver *s) {
+    int f = 0;
+    CU(cudaMemcpyAsync(&f, s->flag, sizeof(int), cudaMemcpyDeviceToHost, s->stream));
+    CU(cudaStreamSynchronize(s->stream));
+    if (f) return fail(DG_EUNPHYSICAL, "rho <= 0 or p <= 0 at an evaluation point%s");
+    return DG_OK;
+}
+
+void drop_graph(dg_solver *s) {
+    if (s->graph) {
+        cudaGraphExecDestroy(s->graph);
+        s->graph = nullptr;
+    }
+}
+
+int init_common(dg_solver **out, const dg_mesh *mesh, int order, double gamma, double nu, double chi,
+                const dg_options *opt, void *ws, size_t ws_bytes, size_t *need_only) {
+    dg_options o;
+    dg_default_options(&o);
+    if (opt) o = *opt;
+    int rc = validate(mesh, order, gamma, nu, chi, &o);
+    if (rc) return rc;
+    dg_solver *s = new (std::nothrow) dg_solver();
+    if (!s) return fail(DG_ENOMEM, "host allocation failed");
+    std::memset(s, 0, sizeof(*s));
+    s->dim = mesh->dim;
+    s->order = order;
+    s->ncells = 1;
+    for (int a = 0; a < 3; ++a) {
+        s->ncell[a] = (a < mesh->dim) ? mesh->ncell[a] : 1;
+        s->ncells *= s->ncell[a];
+    }
+    s->h = mesh->h;
+    s->gamma = gamma;
+    s->nu = nu;
+    s->chi = chi;
+    s->opt = o;
+    s->visc = (nu > 0.0 || chi > 0.0) ? 1 : 0;
+    s->av = o.av_enable ? 1 : 0;
+    s->Vc = s->dim + 2;
+    s->V = s->Vc + s->av;
+    s->M = 1;
+    for (int a = 0; a < s->dim; ++a) s->M *= order;
+    s->nstate = (size_t)s->V * s->M * s->ncells;
+    s->fn = kDispatch[s->dim - 2][order - 1];
+    const size_t need = workspace_layout(s, nullptr);
+    if (need_only) {
+        *need_only = need;
+        delete s;
+        return DG_OK;
+    }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        delete s;
+        return fail(DG_ECUDA, "no CUDA device: this library has no CPU path%s");
+    }
+    char *base = (char *)ws;
+    if (base) {
+        if (ws_bytes < need || ((size_t)base & 255)) {
+            delete s;
+            return fail(DG_EINVAL, "workspace too small or not 256-byte aligned");
+        }
+    } else {
+        if (cudaMalloc((void **)&base, need) != cudaSuccess) {
+            cudaGetLastError();
+            delete s;
+            return fail(DG_ENOMEM, "cudaMalloc of the solver state failed");
+        }
+        s->owned = base;
+    }
+    workspace_layout(s, base);
+    cudaError_t e = s->fn.config(s->visc, s->av);
+    if (e == cudaSuccess) {
+        DgTables t;
+        dg_build_tables(order, &t);
+        e = s->fn.upload(&t);
+    }
+    if (e == cudaSuccess) e = cudaMemset(base, 0, need);
+    if (e != cudaSuccess) {
+        if (s->owned) cudaFree(s->owned);
+        delete s;
+        return fail(DG_ECUDA, "kernel configuration failed (needs an sm_100a device): %s", cudaGetErrorString(e));
+    }
+    s->fn.info(s->visc, s->av, &s->kC, &s->kNT, &s->kSmem);
+    *out = s;
+    return DG_OK;
+}
+
+// copy between a caller buffer with `nv` variables per mode and the internal V-variable layout
+int copy_vars(dg_solver *s, void *dst, size_t dpitch_vars, const void *src, size_t spitch_vars, size_t nv) {
+    const size_t row = (size_t)s->ncells * sizeof(double);
+    CU(cudaMemcpy2DAsync(dst, dpitch_vars * row, src, spitch_vars * row, nv * row, s->M, cudaMemcpyDefault,
+                         s->stream));
+    return DG_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int dg_default_options(dg_options *opt) {
+    if (!opt) return fail(DG_EINVAL, "opt is NULL");
+    opt->f_cfl = 0.5;
+    opt->rk_stages = 3;
+    opt->av_enable = 0;
+    opt->f_v = 2.5;
+    opt->f_tau = 0.5;
+    opt->f_w = 0.2;
+    opt->s_onset0 = 1.0e-4;
+    opt->alpha_max = 1.0;
+    opt->fixed_dt = 0.0;
+    opt->use_graph = 1;
+    return DG_OK;
+}
+
+int dg_init(dg_solver **out, const dg_mesh *mesh, int order, double gamma, double nu, double chi,
+            const dg_options *opt) {
+    if (!out) return fail(DG_EINVAL, "out is NULL");
+    *out = nullptr;
+    return init_common(out, mesh, order, gamma, nu, chi, opt, nullptr, 0, nullptr);
+}
+
+int dg_workspace_bytes(const dg_mesh *mesh, int order, const dg_options *opt, size_t *bytes) {
+    if (!bytes) return fail(DG_EINVAL, "bytes is NULL");
+    return init_common(nullptr, mesh, order, 1.4, 0.0, 0.0, opt, nullptr, 0, bytes);
+}
+
+int dg_init_workspace(dg_solver **out, const dg_mesh *mesh, int order, double gamma, double nu, double chi,
+                      const dg_options *opt, void *device_workspace, size_t bytes) {
+    if (!out) return fail(DG_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (!device_workspace) return fail(DG_EINVAL, "device_workspace is NULL");
+    return init_common(out, mesh, order, gamma, nu, chi, opt, device_workspace, bytes, nullptr);
+}
+
+int dg_set_stream(dg_solver *s, void *cuda_stream) {
+    if (!s) return fail(DG_EINVAL, "solver is NULL");
+    if ((cudaStream_t)cuda_stream != s->stream) drop_graph(s);
+    s->stream = (cudaStream_t)cuda_stream;
+    return DG_OK;
+}
+
+int dg_set_state(dg_solver *s, const double *w, size_t count) {
+    if (!s || !w) return fail(DG_EINVAL, "NULL argument");
+    if (count != (size_t)s->Vc * s->M * s->ncells) return fail(DG_EINVAL, "count must be Vc*M*Ncells");
+    CU(cudaMemsetAsync(s->W0, 0, s->nstate * sizeof(double), s->stream));
+    int rc = copy_vars(s, s->W0, s->V, w, s->Vc, s->Vc);
+    if (rc) return rc;
+    if (s->av) {
+        CU(cudaMemsetAsync(s->sens_prev, 0, 2 * (size_t)s->ncells * sizeof(double), s->stream));
+        CU(cudaMemsetAsync(s->sens_new, 0, 2 * (size_t)s->ncells * sizeof(double), s->stream));
+    }
+    CU(cudaMemsetAsync(s->scal, 0, 16 * sizeof(double), s->stream));
+    CU(cudaMemsetAsync(s->flag, 0, sizeof(int), s->stream));
+    rc = enqueue_wavespeed(s);
+    if (rc) return rc;
+    CU(cudaStreamSynchronize(s->stream));   // the caller's buffer may be pageable / reused
+    return DG_OK;
+}
+
+int dg_set_alpha(dg_solver *s, const double *alpha, size_t count) {
+    if (!s || !alpha) return fail(DG_EINVAL, "NULL argument");
+    if (!s->av) return fail(DG_EINVAL, "artificial viscosity is not enabled");
+    if (count != (size_t)s->M * s->ncells) return fail(DG_EINVAL, "count must be M*Ncells");
+    int rc = copy_vars(s, s->W0 + (size_t)s->Vc * s->ncells, s->V, alpha, 1, 1);
+    if (rc) return rc;
+    CU(cudaStreamSynchronize(s->stream));
+    return DG_OK;
+}
+
+int dg_step_async(dg_solver *s, int nsteps) {
+    if (!s) return fail(DG_EINVAL, "solver is NULL");
+    if (nsteps < 0) return fail(DG_EINVAL, "nsteps must be >= 0");
+    if (!s->speeds_valid) {
+        int rc = enqueue_wavespeed(s);
+        if (rc) return rc;
+    }
+    const int per_step = 1 + s->opt.rk_stages;
+    if (s->opt.use_graph && nsteps > 0) {
+        if (!s->graph) {
+            cudaStream_t cap = s->stream;
+            cudaStream_t tmp = nullptr;
+            if (cap == nullptr || cap == cudaStreamLegacy) {   // the legacy stream cannot be captured
+                CU(cudaStreamCreateWithFlags(&tmp, cudaStreamNonBlocking));
+                cap = tmp;
+            }
+            cudaStream_t keep = s->stream;
+            s->stream = cap;
+            cudaGraph_t g = nullptr;
+            cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
+            int rc = DG_OK;
+            if (e == cudaSuccess) {
+                rc = enqueue_step(s);
+                e = cudaStreamEndCapture(cap, &g);
+            }
+            s->stream = keep;
+            if (tmp) cudaStreamDestroy(tmp);
+            if (rc) return rc;
+            if (e != cudaSuccess) return fail(DG_ECUDA, "graph capture failed: %s", cudaGetErrorString(e));
+            e = cudaGraphInstantiate(&s->graph, g, 0);
+            cudaGraphDestroy(g);
+            if (e != cudaSuccess) return fail(DG_ECUDA, "cudaGraphInstantiate: %s", cudaGetErrorString(e));
+        }
+        for (int k = 0; k < nsteps; ++k) CU(cudaGraphLaunch(s->graph, s->stream));
+    } else {
+        for (int k = 0; k < nsteps; ++k) {
+            int rc = enqueue_step(s);
+            if (rc) return rc;
+        }
+    }
+    s->launches += (long long)nsteps * per_step;
+    return DG_OK;
+}
+
+int dg_sync(dg_solver *s) {
+    if (!s) return fail(DG_EINVAL, "solver is NULL");
+    return check_flag(s);
+}
+
+int dg_step(dg_solver *s, int nsteps) {
+    int rc = dg_step_async(s, nsteps);
+    if (rc) return rc;
+    return check_flag(s);
+}
+
+int dg_get_state(dg_solver *s, double *w, size_t count) {
+    if (!s || !w) return fail(DG_EINVAL, "NULL argument");
+    if (count != (size_t)s->Vc * s->M * s->ncells) return fail(DG_EINVAL, "count must be Vc*M*Ncells");
+    int rc = copy_vars(s, w, s->Vc, s->W0, s->V, s->Vc);
+    if (rc) return rc;
+    CU(cudaStreamSynchronize(s->stream));
+    return DG_OK;
+}
+
+int dg_get_alpha(dg_solver *s, double *alpha, size_t count) {
+    if (!s || !alpha) return fail(DG_EINVAL, "NULL argument");
+    if (count != (size_t)s->M * s->ncells) return fail(DG_EINVAL, "count must be M*Ncells");
+    if (!s->av) {
+        cudaPointerAttributes at;
+        if (cudaPointerGetAttributes(&at, alpha) == cudaSuccess && at.type == cudaMemoryTypeDevice) {
+            CU(cudaMemsetAsync(alpha, 0, count * sizeof(double), s->stream));
+            CU(cudaStreamSynchronize(s->stream));
+        } else {
+            cudaGetLastError();
+            std::memset(alpha, 0, count * sizeof(double));
+        }
+        return DG_OK;
+    }
+    int rc = copy_vars(s, alpha, 1, s->W0 + (size_t)s->Vc * s->ncells, s->V, 1);
+    if (rc) return rc;
+    CU(cudaStreamSynchronize(s->stream));
+    return DG_OK;
+}
+
+int dg_conserved_totals(dg_solver *s, double totals[5]) {
+    if (!s || !totals) return fail(DG_EINVAL, "NULL argument");
+    double vol = 1.0;
+    for (int a = 0; a < s->dim; ++a) vol *= s->h;
+    dg_totals_kernel<<<s->Vc, 1024, 0, s->stream>>>(s->W0, s->V, s->ncells, vol, s->scal + 8);
+    CU(cudaGetLastError());
+    s->launches += 1;
+    double t[5] = {0, 0, 0, 0, 0};
+    CU(cudaMemcpyAsync(t, s->scal + 8, s->Vc * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    CU(cudaStreamSynchronize(s->stream));
+    for (int i = 0; i < 5; ++i) totals[i] = (i < s->Vc) ? t[i] : 0.0;
+    return DG_OK;
+}
+
+int dg_eval_rhs(dg_solver *s, double *out, size_t count, double *alpha_out, size_t alpha_count) {
+    if (!s || !out) return fail(DG_EINVAL, "NULL argument");
+    if (count != (size_t)s->Vc * s->M * s->ncells) return fail(DG_EINVAL, "count must be Vc*M*Ncells");
+    if (alpha_out && alpha_count != (size_t)s->M * s->ncells) return fail(DG_EINVAL, "alpha_count must be M*Ncells");
+    DgStageArgs a;
+    fill_args(s, &a);
+    a.w_prev = s->W0;
+    a.w_n = s->W0;
+    a.w_out = s->WA;
+    a.rhs_only = 1;
+    CU(s->fn.launch(s->visc, s->av, &a, s->stream, 0));
+    s->launches += 1;
+    int rc = copy_vars(s, out, s->Vc, s->WA, s->V, s->Vc);
+    if (rc) return rc;
+    if (alpha_out) {
+        if (s->av) {
+            rc = copy_vars(s, alpha_out, 1, s->WA + (size_t)s->Vc * s->ncells, s->V, 1);
+            if (rc) return rc;
+        } else {
+            CU(cudaStreamSynchronize(s->stream));
+            std::memset(alpha_out, 0, alpha_count * sizeof(double));
+        }
+    }
+    return check_flag(s);
+}
+
+int dg_get_time(dg_solver *s, double *t, double *last_dt) {
+    if (!s) return fail(DG_EINVAL, "solver is NULL");
+    double v[2];
+    CU(cudaMemcpyAsync(v, s->scal, 2 * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    CU(cudaStreamSynchronize(s->stream));
+    if (last_dt) *last_dt = v[0];
+    if (t) *t = v[1];
+    return DG_OK;
+}
+
+int dg_kernel_info(dg_solver *s, int *cells_per_block, int *threads, int *smem_bytes, int *blocks) {
+    if (!s) return fail(DG_EINVAL, "solver is NULL");
+    if (cells_per_block) *cells_per_block = s->kC;
+    if (threads) *threads = s->kNT;
+    if (smem_bytes) *smem_bytes = s->kSmem;
+    if (blocks) *blocks = (s->ncells + s->kC - 1) / s->kC;
+    return DG_OK;
+}
+
+int dg_launch_count(dg_solver *s, long long *count) {
+    if (!s || !count) return fail(DG_EINVAL, "NULL argument");
+    *count = s->launches;
+    return DG_OK;
+}
+
+int dg_measure_fp64_peak(int iters, double *flops_per_s, void *cuda_stream) {
+    if (!flops_per_s || iters < 1) return fail(DG_EINVAL, "bad argument");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return fail(DG_ECUDA, "no CUDA device%s");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    cudaDeviceProp prop;
+    int dev = 0;
+    CU(cudaGetDevice(&dev));
+    CU(cudaGetDeviceProperties(&prop, dev));
+    double *d = nullptr;
+    CU(cudaMalloc(&d, sizeof(double)));
+    const int blocks = prop.multiProcessorCount * 8;
+    cudaEvent_t e0, e1;
+    CU(cudaEventCreate(&e0));
+    CU(cudaEventCreate(&e1));
+    dg_dfma_kernel<<<blocks, 256, 0, st>>>(d, iters / 4 + 1, 1.0, 0.0);
+    CU(cudaEventRecord(e0, st));
+    dg_dfma_kernel<<<blocks, 256, 0, st>>>(d, iters, 1.0, 0.0);
+    CU(cudaEventRecord(e1, st));
+    CU(cudaEventSynchronize(e1));
+    float ms = 0.f;
+    CU(cudaEventElapsedTime(&ms, e0, e1));
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(d);
+    const double flops = 2.0 * 64.0 * (double)iters * 256.0 * (double)blocks;
+    *flops_per_s = flops / (ms * 1e-3);
+    return DG_OK;
+}
+
+int dg_free(dg_solver *s) {
+    if (!s) return DG_OK;
+    drop_graph(s);
+    if (s->owned) cudaFree(s->owned);
+    delete s;
+    return DG_OK;
+}
+
+const char *dg_last_error(void) { return g_err; }
+
+}  // extern "C"

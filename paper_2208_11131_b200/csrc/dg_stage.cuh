@@ -1,0 +1,676 @@
+// Fused Runge-Kutta-stage kernel of the modal DG operator (sm_100a, fp64 CUDA cores).
+//
+// One launch = one SSP-RK stage over the whole mesh (Eq. 20-21, 200): every thread block
+// owns C consecutive cells and, for each of them, gathers the cell's own modes and its 2d neighbours'
+// modes, evaluates the surface term of Eq. 20 (face traces, HLLC PAPER.md:106, recovery-based viscous /
+// artificial-viscosity face flux PAPER.md:252-305), the volume term (Eq. 21 expansion by sum factorisation,
+// Euler / Navier-Stokes / AV flux, weak-form derivative, projection), the stage combine and -- on the last
+// stage -- the wave-speed maxima of Eq. 23 for the next step.  dw/dt never touches HBM.
+//
+// Shared-memory layout per block (doubles):  [slot][point][cell], cell fastest (C cells), so that a warp
+// whose lanes are consecutive cells reads/writes conflict-free and global accesses coalesce along `cell`
+// (state layout w[(mode*V + var)*Ncells + cell]).
+//   RA   V  x Np   own modes  -> nodal values (in place)
+//   RX   max(D*Vc*Np, 2*NQ*Nf)   face scratch (one axis, both faces)  /  gradients -> fluxes (in place)
+//   ACC  V  x Np   dw/dt in modal space
+// No float atomics, no races: each cell's dw/dt is a fixed-order gather (bit-reproducible run to run).
+#pragma once
+
+#include <cuda_runtime.h>
+
+#include "dg_tables.h"
+
+#include "dg_stage_args.h"
+
+#define DG_SEL_V 0
+#define DG_SEL_DHAT 1
+#define DG_SEL_S 2
+#define DG_SEL_VTG 3
+
+__constant__ DgTables c_tab;
+
+namespace dgk {
+
+__host__ __device__ constexpr int ipow(int b, int e) { return e <= 0 ? 1 : b * ipow(b, e - 1); }
+__host__ __device__ constexpr int imax(int a, int b) { return a > b ? a : b; }
+
+constexpr int kSmemBudget = 112 * 1024;   // two resident blocks per SM (228 KB, 1 KB reserved per block)
+constexpr int kSmemMax = 227 * 1024;
+
+template <int D, int M, bool VISC, bool AV>
+struct Cfg {
+    static constexpr bool GRAD = VISC || AV;
+    static constexpr int Vc = D + 2;
+    static constexpr int V = Vc + (AV ? 1 : 0);
+    static constexpr int Np = ipow(M, D);
+    static constexpr int Nf = ipow(M, D - 1);
+    // face scratch slots per side: uL(Vc) uR(Vc) [u~(V) gn(Vc) gt((D-1) Vc)]
+    static constexpr int NQE = GRAD ? (3 * Vc + V) : 2 * Vc;      // slots expanded modal -> nodal
+    static constexpr int NQ = NQE + (GRAD ? (D - 1) * Vc : 0);
+    static constexpr int RX = imax(D * Vc * Np, 2 * NQ * Nf);
+    static constexpr int FP = 2 * V * Np + RX;                     // doubles per cell
+    static constexpr int NT = 256;
+    static constexpr int pick_c() {
+        int c = 32;
+        while (c > 1 && c * FP * 8 > kSmemBudget) c >>= 1;
+        return c;
+    }
+    static constexpr int C = pick_c();
+    static constexpr int kExtraDoubles = C + 2 * (NT / 32);        // W^K per cell, reduction scratch
+    static constexpr int kSmemBytes = (C * FP + kExtraDoubles) * 8 + 2 * D * C * 4;
+    static_assert(kSmemBytes <= kSmemMax, "per-cell footprint exceeds shared memory");
+};
+
+template <int SEL>
+__device__ __forceinline__ double mat(int idx) {
+    if (SEL == DG_SEL_V) return c_tab.V[idx];
+    if (SEL == DG_SEL_DHAT) return c_tab.Dhat[idx];
+    if (SEL == DG_SEL_S) return c_tab.S[idx];
+    return c_tab.VtG[idx];
+}
+
+// pencil base: index of the first point of pencil `pen` along an axis of stride STRIDE
+template <int M, int STRIDE>
+__device__ __forceinline__ int pencil_base(int pen) {
+    return (pen / STRIDE) * (STRIDE * M) + (pen % STRIDE);
+}
+
+// Apply one 1D matrix along one axis to `nslots` arrays of NPTS points:
+//   dst[slot][p] (+)= scale * sum_i MAT[j][i] * (sum_{k<NSUM} src[k*sum_stride + slot][p_i])
+// src == dst (in place) is allowed: a thread owns whole pencils.
+template <int SEL, int M, int NPTS, int STRIDE, int C, int NT, int NSUM, bool ADD, bool SCALE>
+__device__ __forceinline__ void sweep(const double *src, int sum_stride, double *dst, int nslots, double scale,
+                                      int tid) {
+    constexpr int NPEN = NPTS / M;
+    const int total = nslots * NPEN * C;
+    for (int it = tid; it < total; it += NT) {
+        const int cell = it % C;
+        const int r = it / C;
+        const int pen = r % NPEN;
+        const int slot = r / NPEN;
+        const int off = (slot * NPTS + pencil_base<M, STRIDE>(pen)) * C + cell;
+        double in[M];
+#pragma unroll
+        for (int i = 0; i < M; ++i) {
+            in[i] = src[off + i * STRIDE * C];
+#pragma unroll
+            for (int k = 1; k < NSUM; ++k) in[i] += src[k * sum_stride + off + i * STRIDE * C];
+        }
+#pragma unroll
+        for (int j = 0; j < M; ++j) {
+            double acc = mat<SEL>(j * 8) * in[0];
+#pragma unroll
+            for (int i = 1; i < M; ++i) acc = fma(mat<SEL>(j * 8 + i), in[i], acc);
+            if (SCALE) acc *= scale;
+            if (ADD)
+                dst[off + j * STRIDE * C] += acc;
+            else
+                dst[off + j * STRIDE * C] = acc;
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// point-wise physics (Eq. 1-5; 106; 311-323 Eq. 37-39; 375-407 Eq. 43-46)
+// ---------------------------------------------------------------------------------------------------
+template <int D>
+struct Prim {
+    double rho, ir, v[D], p, e;
+};
+
+template <int D>
+__device__ __forceinline__ Prim<D> primitives(const double *u, double gamma) {
+    Prim<D> q;
+    q.rho = u[0];
+    q.ir = 1.0 / q.rho;
+    double v2 = 0.0;
+#pragma unroll
+    for (int b = 0; b < D; ++b) {
+        q.v[b] = u[1 + b] * q.ir;
+        v2 = fma(q.v[b], q.v[b], v2);
+    }
+    q.e = u[1 + D];
+    q.p = (gamma - 1.0) * (q.e - 0.5 * q.rho * v2);
+    return q;
+}
+
+// Euler flux along axis a (Eq. 4; energy row (e+p) v_a, reading A5)
+template <int D>
+__device__ __forceinline__ void euler_flux(const double *u, const Prim<D> &q, int a, double *f) {
+    const double va = q.v[a];
+    f[0] = u[1 + a];
+#pragma unroll
+    for (int b = 0; b < D; ++b) f[1 + b] = u[1 + a] * q.v[b] + (b == a ? q.p : 0.0);
+    f[1 + D] = (q.e + q.p) * va;
+}
+
+// HLLC flux along axis a (Toro's HLLC with Davis wave-speed bounds, reading A6)
+template <int D>
+__device__ __forceinline__ void hllc_flux(const double *uL, const double *uR, const Prim<D> &L, const Prim<D> &R,
+                                          int a, double gamma, double *F) {
+    const double cL = sqrt(gamma * L.p * L.ir);
+    const double cR = sqrt(gamma * R.p * R.ir);
+    const double vnL = L.v[a], vnR = R.v[a];
+    const double SL = fmin(vnL - cL, vnR - cR);
+    const double SR = fmax(vnL + cL, vnR + cR);
+    if (SL >= 0.0) {
+        euler_flux<D>(uL, L, a, F);
+        return;
+    }
+    if (SR <= 0.0) {
+        euler_flux<D>(uR, R, a, F);
+        return;
+    }
+    const double mL = L.rho * (SL - vnL);
+    const double mR = R.rho * (SR - vnR);
+    const double Sstar = (R.p - L.p + mL * vnL - mR * vnR) / (mL - mR);
+    // F_K + S_K (U*_K - U_K), K = L if S* >= 0 else R
+    const bool left = (Sstar >= 0.0);
+    const double *u = left ? uL : uR;
+    const Prim<D> &K = left ? L : R;
+    const double S = left ? SL : SR;
+    const double vn = left ? vnL : vnR;
+    const double mK = left ? mL : mR;
+    double f[D + 2];
+    euler_flux<D>(u, K, a, f);
+    const double fac = mK / (S - Sstar);
+    F[0] = f[0] + S * (fac - u[0]);
+#pragma unroll
+    for (int b = 0; b < D; ++b) {
+        const double us = fac * (b == a ? Sstar : K.v[b]);
+        F[1 + b] = f[1 + b] + S * (us - u[1 + b]);
+    }
+    const double es = fac * (K.e * K.ir + (Sstar - vn) * (Sstar + K.p / mK));
+    F[1 + D] = f[1 + D] + S * (es - K.e);
+}
+
+// velocity gradient dv[b][c] = d v_c / d x_b = (d_b(rho v_c) - v_c d_b rho) / rho
+template <int D>
+__device__ __forceinline__ void velocity_gradient(const Prim<D> &q, const double (*g)[D + 2], double (*dv)[D]) {
+#pragma unroll
+    for (int b = 0; b < D; ++b)
+#pragma unroll
+        for (int c = 0; c < D; ++c) dv[b][c] = (g[b][1 + c] - q.v[c] * g[b][0]) * q.ir;
+}
+
+// Navier-Stokes flux column a (Eq. 38-39, traceless Pi, reading A7), SUBTRACTED from F
+template <int D>
+__device__ __forceinline__ void ns_flux_sub(const Prim<D> &q, const double (*g)[D + 2], const double (*dv)[D],
+                                            double divv, int a, double gamma, double nu, double chi, double *F) {
+    double evisc = 0.0;
+#pragma unroll
+    for (int b = 0; b < D; ++b) {
+        const double Pi = nu * q.rho * (dv[a][b] + dv[b][a] - (a == b ? (2.0 / 3.0) * divv : 0.0));
+        F[1 + b] -= Pi;
+        evisc = fma(q.v[b], Pi, evisc);
+    }
+    double vdv = 0.0;
+#pragma unroll
+    for (int c = 0; c < D; ++c) vdv = fma(q.v[c], dv[a][c], vdv);
+    const double duth = g[a][1 + D] * q.ir - q.e * g[a][0] * (q.ir * q.ir) - vdv;
+    F[1 + D] -= evisc + chi * (gamma - 1.0) * q.rho * duth;
+}
+
+__device__ __forceinline__ void atomic_max_nonneg(unsigned long long *addr, double val) {
+    atomicMax(addr, (unsigned long long)__double_as_longlong(val));
+}
+
+// block-wide max of two non-negative values -> atomicMax on maxbits[0..1]
+template <int NT>
+__device__ __forceinline__ void block_max2(double a, double b, double *red, unsigned long long *maxbits, int tid) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        a = fmax(a, __shfl_xor_sync(0xffffffffu, a, o));
+        b = fmax(b, __shfl_xor_sync(0xffffffffu, b, o));
+    }
+    if ((tid & 31) == 0) {
+        red[tid >> 5] = a;
+        red[NT / 32 + (tid >> 5)] = b;
+    }
+    __syncthreads();
+    if (tid == 0) {
+        for (int i = 1; i < NT / 32; ++i) {
+            a = fmax(a, red[i]);
+            b = fmax(b, red[NT / 32 + i]);
+        }
+        atomic_max_nonneg(&maxbits[0], a);
+        atomic_max_nonneg(&maxbits[1], b);
+    }
+}
+
+// expand slots [0, nslots) of `buf` modal -> nodal in place (Eq. 21), all D axes; ends with a barrier
+template <int D, int M, int C, int NT>
+__device__ __forceinline__ void expand_volume(double *buf, int nslots, int tid) {
+    constexpr int Np = ipow(M, D);
+    sweep<DG_SEL_V, M, Np, 1, C, NT, 1, false, false>(buf, 0, buf, nslots, 1.0, tid);
+    __syncthreads();
+    sweep<DG_SEL_V, M, Np, M, C, NT, 1, false, false>(buf, 0, buf, nslots, 1.0, tid);
+    __syncthreads();
+    if (D == 3) {
+        sweep<DG_SEL_V, M, Np, M * M, C, NT, 1, false, false>(buf, 0, buf, nslots, 1.0, tid);
+        __syncthreads();
+    }
+}
+
+// max c_s and max |v| over the nodal values in RA (Eq. 23 inputs, reading A18)
+template <int D, int M, int C, int NT>
+__device__ __forceinline__ void wavespeed_points(const double *RA, double gamma, int *flag, double *red,
+                                                 unsigned long long *maxbits, int tid) {
+    constexpr int Np = ipow(M, D);
+    constexpr int Vc = D + 2;
+    double cmax = 0.0, vmax = 0.0;
+    bool bad = false;
+    for (int it = tid; it < Np * C; it += NT) {
+        const int cell = it % C;
+        const int j = it / C;
+        double u[Vc];
+#pragma unroll
+        for (int v = 0; v < Vc; ++v) u[v] = RA[(v * Np + j) * C + cell];
+        const Prim<D> q = primitives<D>(u, gamma);
+        bad |= !(q.rho > 0.0) || !(q.p > 0.0);
+        double v2 = 0.0;
+#pragma unroll
+        for (int b = 0; b < D; ++b) v2 = fma(q.v[b], q.v[b], v2);
+        const double cs = sqrt(gamma * q.p * q.ir);
+        const double vm = sqrt(v2);
+        cmax = (cs > cmax) ? cs : cmax;   // NaN-safe: NaN never becomes the maximum
+        vmax = (vm > vmax) ? vm : vmax;
+    }
+    if (bad) atomicOr(flag, 1);
+    block_max2<NT>(cmax, vmax, red, maxbits, tid);
+}
+
+// ---------------------------------------------------------------------------------------------------
+// surface term of Eq. 20 for axis A: both faces of every cell of the block (gather form)
+// ---------------------------------------------------------------------------------------------------
+template <int D, int M, bool VISC, bool AV, int A>
+__device__ __forceinline__ void face_axis(const DgStageArgs &p, double *RA, double *RX, double *ACC,
+                                          const int *nbr, int tid) {
+    using K = Cfg<D, M, VISC, AV>;
+    constexpr int C = K::C, NT = K::NT, V = K::V, Vc = K::Vc, Np = K::Np, Nf = K::Nf, NQ = K::NQ;
+    constexpr bool GRAD = K::GRAD;
+    constexpr int SA = ipow(M, A);               // stride of axis A inside the cell
+    constexpr int SIDE = NQ * Nf * C;            // doubles per face side in RX
+    constexpr int oUL = 0, oUR = Vc, oUT = 2 * Vc, oGN = 2 * Vc + V, oGT = 3 * Vc + V;
+    const double ih = 1.0 / p.h;
+
+    // F1: contract the normal axis (PAPER.md:171 traces; 294-299 recovery partial sums)
+    for (int it = tid; it < 2 * V * Nf * C; it += NT) {
+        const int cell = it % C;
+        int r = it / C;
+        const int lt = r % Nf;
+        r /= Nf;
+        const int v = r % V;
+        const int s = r / V;   // 0: face towards -A (neighbour is the LEFT state), 1: face towards +A
+        const int base = pencil_base<M, SA>(lt);
+        const int nc = nbr[(2 * A + s) * C + cell];
+        double own[M], nb[M];
+#pragma unroll
+        for (int l = 0; l < M; ++l) nb[l] = p.w_prev[(size_t)((base + l * SA) * V + v) * p.ncells + nc];
+#pragma unroll
+        for (int l = 0; l < M; ++l) own[l] = RA[(v * Np + base + l * SA) * C + cell];
+        double *F = RX + s * SIDE + lt * C + cell;
+        double uL = 0.0, uR = 0.0, ut = 0.0, gn = 0.0;
+#pragma unroll
+        for (int l = 0; l < M; ++l) {
+            const double lf = s ? own[l] : nb[l];
+            const double rt = s ? nb[l] : own[l];
+            uL = fma(c_tab.Pend[1][l], lf, uL);
+            uR = fma(c_tab.Pend[0][l], rt, uR);
+            if (GRAD) {
+                ut = fma(c_tab.Rv[0][l], lf, ut);
+                ut = fma(c_tab.Rv[1][l], rt, ut);
+                gn = fma(c_tab.Gv[0][l], lf, gn);
+                gn = fma(c_tab.Gv[1][l], rt, gn);
+            }
+        }
+        if (v < Vc) {
+            F[(oUL + v) * Nf * C] = uL;
+            F[(oUR + v) * Nf * C] = uR;
+            if (GRAD) F[(oGN + v) * Nf * C] = gn * ih;
+        }
+        if (GRAD) F[(oUT + v) * Nf * C] = ut;
+    }
+    __syncthreads();
+
+    // F2: transverse modal -> nodal on the face (cell basis kept transversally)
+    if (M > 1) {
+#pragma unroll
+        for (int s = 0; s < 2; ++s)
+            sweep<DG_SEL_V, M, Nf, 1, C, NT, 1, false, false>(RX + s * SIDE, 0, RX + s * SIDE, K::NQE, 1.0, tid);
+        __syncthreads();
+        if (D == 3) {
+#pragma unroll
+            for (int s = 0; s < 2; ++s)
+                sweep<DG_SEL_V, M, Nf, M, C, NT, 1, false, false>(RX + s * SIDE, 0, RX + s * SIDE, K::NQE, 1.0, tid);
+            __syncthreads();
+        }
+    }
+    if (GRAD) {
+        // transverse derivatives of the recovered face polynomial
+#pragma unroll
+        for (int s = 0; s < 2; ++s) {
+            sweep<DG_SEL_DHAT, M, Nf, 1, C, NT, 1, false, true>(RX + s * SIDE + oUT * Nf * C, 0,
+                                                               RX + s * SIDE + oGT * Nf * C, Vc, 2.0 * ih, tid);
+            if (D == 3)
+                sweep<DG_SEL_DHAT, M, Nf, M, C, NT, 1, false, true>(RX + s * SIDE + oUT * Nf * C, 0,
+                                                                   RX + s * SIDE + (oGT + Vc) * Nf * C, Vc,
+                                                                   2.0 * ih, tid);
+        }
+        __syncthreads();
+    }
+
+    // F3: numerical flux at every face point; result overwrites the uL slots
+    {
+        bool bad = false;
+        for (int it = tid; it < 2 * Nf * C; it += NT) {
+            const int cell = it % C;
+            const int r = it / C;
+            const int k = r % Nf;
+            const int s = r / Nf;
+            double *F = RX + s * SIDE + k * C + cell;
+            double uL[Vc], uR[Vc], Fh[Vc];
+#pragma unroll
+            for (int v = 0; v < Vc; ++v) {
+                uL[v] = F[(oUL + v) * Nf * C];
+                uR[v] = F[(oUR + v) * Nf * C];
+            }
+            const Prim<D> qL = primitives<D>(uL, p.gamma);
+            const Prim<D> qR = primitives<D>(uR, p.gamma);
+            bad |= !(qL.rho > 0.0) || !(qL.p > 0.0) || !(qR.rho > 0.0) || !(qR.p > 0.0);
+            hllc_flux<D>(uL, uR, qL, qR, A, p.gamma, Fh);
+            if (GRAD) {
+                double ut[Vc], g[D][D + 2];
+#pragma unroll
+                for (int v = 0; v < Vc; ++v) {
+                    ut[v] = F[(oUT + v) * Nf * C];
+#pragma unroll
+                    for (int b = 0; b < D; ++b) {
+                        const int slot = (b == A) ? (oGN + v) : (oGT + (b < A ? b : b - 1) * Vc + v);
+                        g[b][v] = F[slot * Nf * C];
+                    }
+                }
+                const Prim<D> qt = primitives<D>(ut, p.gamma);
+                bad |= !(qt.rho > 0.0) || !(qt.p > 0.0);
+                if (VISC) {
+                    double dv[D][D];
+                    velocity_gradient<D>(qt, g, dv);
+                    double divv = 0.0;
+#pragma unroll
+                    for (int b = 0; b < D; ++b) divv += dv[b][b];
+                    ns_flux_sub<D>(qt, g, dv, divv, A, p.gamma, p.nu, p.chi, Fh);
+                }
+                if (AV) {
+                    const double al = F[(oUT + Vc) * Nf * C];
+                    const double cst = sqrt(p.gamma * qt.p * qt.ir);
+                    const double eps = fmin(fmax(al, 0.0), p.alpha_max) * cst * p.h / (double)M;   // Eq. 46, A12
+#pragma unroll
+                    for (int v = 0; v < Vc; ++v) Fh[v] -= eps * g[A][v];
+                }
+            }
+#pragma unroll
+            for (int v = 0; v < Vc; ++v) F[(oUL + v) * Nf * C] = Fh[v];
+        }
+        if (bad) atomicOr(p.flag, 1);
+    }
+    __syncthreads();
+
+    // F4: project the face flux on the transverse modes (g_k phi_l(xi_k) of Eq. 20's surface lines)
+    if (M > 1) {
+#pragma unroll
+        for (int s = 0; s < 2; ++s)
+            sweep<DG_SEL_VTG, M, Nf, 1, C, NT, 1, false, false>(RX + s * SIDE, 0, RX + s * SIDE, Vc, 1.0, tid);
+        __syncthreads();
+        if (D == 3) {
+#pragma unroll
+            for (int s = 0; s < 2; ++s)
+                sweep<DG_SEL_VTG, M, Nf, M, C, NT, 1, false, false>(RX + s * SIDE, 0, RX + s * SIDE, Vc, 1.0, tid);
+            __syncthreads();
+        }
+    } else {
+        // single point: weight g_0^(D-1) = 2^(D-1)
+        for (int it = tid; it < 2 * Vc * C; it += NT) {
+            const int cell = it % C;
+            const int r = it / C;
+            RX[(r / Vc) * SIDE + (r % Vc) * Nf * C + cell] *= (D == 3 ? 4.0 : 2.0);
+        }
+        __syncthreads();
+    }
+
+    // F5: lift along the normal: dw_l -= pref [P_l(+1) F^(+) - P_l(-1) F^(-)]   (Eq. 20, readings A3/A4)
+    {
+        const double pref = (D == 3 ? 0.25 : 0.5) * ih;
+        for (int it = tid; it < Vc * Nf * C; it += NT) {
+            const int cell = it % C;
+            const int r = it / C;
+            const int lt = r % Nf;
+            const int v = r / Nf;
+            const double Fm = RX[(v * Nf + lt) * C + cell];          // face towards -A
+            const double Fp = RX[SIDE + (v * Nf + lt) * C + cell];   // face towards +A
+            const int base = pencil_base<M, SA>(lt);
+#pragma unroll
+            for (int l = 0; l < M; ++l)
+                ACC[(v * Np + base + l * SA) * C + cell] += pref * (c_tab.Pend[0][l] * Fm - c_tab.Pend[1][l] * Fp);
+        }
+    }
+    __syncthreads();
+}
+
+// ---------------------------------------------------------------------------------------------------
+// the stage kernel
+// ---------------------------------------------------------------------------------------------------
+template <int D, int M, bool VISC, bool AV>
+__global__ void __launch_bounds__(256, 2) dg_stage_kernel(const DgStageArgs p) {
+    using K = Cfg<D, M, VISC, AV>;
+    constexpr int C = K::C, NT = K::NT, V = K::V, Vc = K::Vc, Np = K::Np;
+    constexpr bool GRAD = K::GRAD;
+    extern __shared__ double smem[];
+    double *RA = smem;
+    double *RX = RA + V * Np * C;
+    double *ACC = RX + K::RX * C;
+    double *Wk = ACC + V * Np * C;
+    double *red = Wk + C;
+    int *nbr = reinterpret_cast<int *>(red + 2 * (NT / 32));
+    const int tid = threadIdx.x;
+    const int cell0 = blockIdx.x * C;
+
+    if (tid < C) {
+        const int c = min(cell0 + tid, p.ncells - 1);
+        const int ix = c % p.nx;
+        const int iy = (c / p.nx) % p.ny;
+        const int iz = c / (p.nx * p.ny);
+        nbr[0 * C + tid] = c + ((ix == 0) ? p.nx - 1 : -1);
+        nbr[1 * C + tid] = c + ((ix == p.nx - 1) ? 1 - p.nx : 1);
+        nbr[2 * C + tid] = c + ((iy == 0) ? (p.ny - 1) * p.nx : -p.nx);
+        nbr[3 * C + tid] = c + ((iy == p.ny - 1) ? -(p.ny - 1) * p.nx : p.nx);
+        if (D == 3) {
+            const int pl = p.nx * p.ny;
+            nbr[(2 * (D - 1)) * C + tid] = c + ((iz == 0) ? (p.nz - 1) * pl : -pl);
+            nbr[(2 * (D - 1) + 1) * C + tid] = c + ((iz == p.nz - 1) ? -(p.nz - 1) * pl : pl);
+        }
+        if (AV) {
+            // wiggle source of Eq. 45 from the previous step's sensor (readings A14, A15)
+            const double S = p.sens_prev[c];
+            const double G = p.sens_prev[p.ncells + c];
+            Wk[tid] = (S > p.s_onset) ? p.f_w * fmax(0.0, G) : 0.0;
+        }
+    }
+    // own modes -> RA, zero ACC
+    for (int it = tid; it < V * Np * C; it += NT) {
+        const int cell = it % C;
+        const int r = it / C;              // global slot order: mode*V + v
+        const int mode = r / V, v = r % V;
+        const int cg = min(cell0 + cell, p.ncells - 1);
+        RA[(v * Np + mode) * C + cell] = p.w_prev[(size_t)r * p.ncells + cg];
+        ACC[it] = 0.0;
+    }
+    __syncthreads();
+
+    // ---- surface term ----
+    face_axis<D, M, VISC, AV, 0>(p, RA, RX, ACC, nbr, tid);
+    face_axis<D, M, VISC, AV, 1>(p, RA, RX, ACC, nbr, tid);
+    if (D == 3) face_axis<D, M, VISC, AV, (D == 3 ? 2 : 0)>(p, RA, RX, ACC, nbr, tid);
+
+    // ---- volume term ----
+    expand_volume<D, M, C, NT>(RA, V, tid);                       // V1: Eq. 21
+    const double ih = 1.0 / p.h;
+    if (GRAD) {
+        // V2: gradients at the Gauss points by analytic differentiation of the basis
+        sweep<DG_SEL_DHAT, M, Np, 1, C, NT, 1, false, true>(RA, 0, RX, Vc, 2.0 * ih, tid);
+        sweep<DG_SEL_DHAT, M, Np, M, C, NT, 1, false, true>(RA, 0, RX + Vc * Np * C, Vc, 2.0 * ih, tid);
+        if (D == 3)
+            sweep<DG_SEL_DHAT, M, Np, M * M, C, NT, 1, false, true>(RA, 0, RX + 2 * Vc * Np * C, Vc, 2.0 * ih, tid);
+        __syncthreads();
+    }
+    {
+        // V3: point-wise fluxes G_a = f_a - F_NS,a - eps d_a u (Eq. 24; 315 Eq. 38), alpha source
+        bool bad = false;
+        for (int it = tid; it < Np * C; it += NT) {
+            const int cell = it % C;
+            const int j = it / C;
+            double u[Vc];
+#pragma unroll
+            for (int v = 0; v < Vc; ++v) u[v] = RA[(v * Np + j) * C + cell];
+            const Prim<D> q = primitives<D>(u, p.gamma);
+            bad |= !(q.rho > 0.0) || !(q.p > 0.0);
+            double g[D][D + 2], dv[D][D];
+            double divv = 0.0, eps = 0.0;
+            if (GRAD) {
+#pragma unroll
+                for (int b = 0; b < D; ++b)
+#pragma unroll
+                    for (int v = 0; v < Vc; ++v) g[b][v] = RX[((b * Vc + v) * Np + j) * C + cell];
+                velocity_gradient<D>(q, g, dv);
+#pragma unroll
+                for (int b = 0; b < D; ++b) divv += dv[b][b];
+            }
+            if (AV) {
+                const double al = RA[(Vc * Np + j) * C + cell];
+                const double cs = sqrt(p.gamma * q.p * q.ir);
+                eps = fmin(fmax(al, 0.0), p.alpha_max) * cs * p.h / (double)M;        // Eq. 46, A17
+                // Eq. 43-45: shock source + wiggle source - decay; stored pre-scaled by h/2 for the projection
+                const double src = p.f_v * fmax(0.0, -divv) + Wk[cell] - al * ((double)M * cs / (p.f_tau * p.h));
+                RA[(Vc * Np + j) * C + cell] = 0.5 * p.h * src;
+            }
+#pragma unroll
+            for (int a = 0; a < D; ++a) {
+                double F[Vc];
+                euler_flux<D>(u, q, a, F);
+                if (VISC) ns_flux_sub<D>(q, g, dv, divv, a, p.gamma, p.nu, p.chi, F);
+                if (AV) {
+#pragma unroll
+                    for (int v = 0; v < Vc; ++v) F[v] -= eps * g[a][v];
+                }
+#pragma unroll
+                for (int v = 0; v < Vc; ++v) RX[((a * Vc + v) * Np + j) * C + cell] = F[v];
+            }
+        }
+        if (bad) atomicOr(p.flag, 1);
+    }
+    __syncthreads();
+    // V4: weak-form derivative in nodal space, N = sum_a S_a G_a
+    sweep<DG_SEL_S, M, Np, 1, C, NT, 1, false, false>(RX, 0, RX, Vc, 1.0, tid);
+    sweep<DG_SEL_S, M, Np, M, C, NT, 1, false, false>(RX + Vc * Np * C, 0, RX + Vc * Np * C, Vc, 1.0, tid);
+    if (D == 3)
+        sweep<DG_SEL_S, M, Np, M * M, C, NT, 1, false, false>(RX + 2 * Vc * Np * C, 0, RX + 2 * Vc * Np * C, Vc, 1.0,
+                                                            tid);
+    __syncthreads();
+    // V5: projection on the modes, dw += pref * (x) VtG N
+    {
+        const double pref = (D == 3 ? 0.25 : 0.5) * ih;
+        sweep<DG_SEL_VTG, M, Np, 1, C, NT, D, false, false>(RX, Vc * Np * C, RX, Vc, 1.0, tid);
+        if (AV) sweep<DG_SEL_VTG, M, Np, 1, C, NT, 1, false, false>(RA + Vc * Np * C, 0, RA + Vc * Np * C, 1, 1.0, tid);
+        __syncthreads();
+        if (D == 3) {
+            sweep<DG_SEL_VTG, M, Np, M, C, NT, 1, false, false>(RX, 0, RX, Vc, 1.0, tid);
+            if (AV)
+                sweep<DG_SEL_VTG, M, Np, M, C, NT, 1, false, false>(RA + Vc * Np * C, 0, RA + Vc * Np * C, 1, 1.0, tid);
+            __syncthreads();
+        }
+        constexpr int SL = (D == 3) ? M * M : M;
+        sweep<DG_SEL_VTG, M, Np, SL, C, NT, 1, true, true>(RX, 0, ACC, Vc, pref, tid);
+        if (AV) sweep<DG_SEL_VTG, M, Np, SL, C, NT, 1, true, true>(RA + Vc * Np * C, 0, ACC + Vc * Np * C, 1, pref, tid);
+        __syncthreads();
+    }
+
+    // ---- sensor bookkeeping (Eq. 42, 45; reading A13/A15): density row of w and dw/dt ----
+    if (AV && p.do_sensor && tid < C && cell0 + tid < p.ncells) {
+        const int c = cell0 + tid;
+        double sA = 0.0, sB = 0.0, dA = 0.0, dB = 0.0;
+        for (int mode = 0; mode < Np; ++mode) {
+            int rem = mode, top = 0;
+#pragma unroll
+            for (int a = 0; a < D; ++a) {
+                top |= (rem % M == M - 1);
+                rem /= M;
+            }
+            const double w = p.w_prev[(size_t)(mode * V) * p.ncells + c];
+            const double wd = ACC[mode * C + tid];
+            sB = fma(w, w, sB);
+            dB = fma(w, wd, dB);
+            if (top && M > 1) {
+                sA = fma(w, w, sA);
+                dA = fma(w, wd, dA);
+            }
+        }
+        p.sens_new[c] = sA / sB;
+        p.sens_new[p.ncells + c] = (sA > 0.0) ? (2.0 * dA / sA - 2.0 * dB / sB) : 0.0;
+    }
+    if (AV && p.commit_sensor && tid < C && cell0 + tid < p.ncells) {
+        const int c = cell0 + tid;
+        p.sens_prev[c] = p.sens_new[c];
+        p.sens_prev[p.ncells + c] = p.sens_new[p.ncells + c];
+    }
+
+    // ---- stage combine ----
+    const double cdt = p.rhs_only ? 1.0 : p.rk_c * p.scal[0];
+    for (int it = tid; it < V * Np * C; it += NT) {
+        const int cell = it % C;
+        const int r = it / C;
+        const int mode = r / V, v = r % V;
+        const int cg = cell0 + cell;
+        const bool active = cg < p.ncells;
+        const size_t gi = (size_t)r * p.ncells + (active ? cg : p.ncells - 1);
+        const double L = ACC[(v * Np + mode) * C + cell];
+        double wnew;
+        if (p.rhs_only) {
+            wnew = L;
+        } else {
+            wnew = p.rk_a * p.w_n[gi];
+            if (p.rk_b != 0.0) wnew = fma(p.rk_b, p.w_prev[gi], wnew);
+            wnew = fma(cdt, L, wnew);
+        }
+        if (active) p.w_out[gi] = wnew;
+        if (p.do_wavespeed) RA[(v * Np + mode) * C + cell] = wnew;
+    }
+    // ---- wave speeds of the new state for the next step's Eq. 23 ----
+    if (p.do_wavespeed) {
+        __syncthreads();
+        expand_volume<D, M, C, NT>(RA, Vc, tid);
+        wavespeed_points<D, M, C, NT>(RA, p.gamma, p.flag, red, p.maxbits, tid);
+    }
+}
+
+// standalone wave-speed kernel (after dg_set_state): load -> expand -> max
+template <int D, int M, bool VISC, bool AV>
+__global__ void __launch_bounds__(256, 2) dg_wavespeed_kernel(const DgStageArgs p) {
+    using K = Cfg<D, M, VISC, AV>;
+    constexpr int C = K::C, NT = K::NT, V = K::V, Vc = K::Vc, Np = K::Np;
+    extern __shared__ double smem[];
+    double *RA = smem;
+    double *red = RA + V * Np * C + K::RX * C + V * Np * C + C;
+    const int tid = threadIdx.x;
+    const int cell0 = blockIdx.x * C;
+    for (int it = tid; it < Vc * Np * C; it += NT) {
+        const int cell = it % C;
+        const int r = it / C;   // mode*Vc + v
+        const int mode = r / Vc, v = r % Vc;
+        const int cg = min(cell0 + cell, p.ncells - 1);
+        RA[(v * Np + mode) * C + cell] = p.w_prev[(size_t)(mode * V + v) * p.ncells + cg];
+    }
+    __syncthreads();
+    expand_volume<D, M, C, NT>(RA, Vc, tid);
+    wavespeed_points<D, M, C, NT>(RA, p.gamma, p.flag, red, p.maxbits, tid);
+}
+
+}  // namespace dgk

@@ -1,0 +1,18 @@
+// Kernel argument block of the fused stage kernel (filled by dg_api.cu, read by dg_stage.cuh).
+#pragma once
+
+struct DgStageArgs {
+    const double *w_prev;   // stage input u^(i-1): halo + own reads
+    const double *w_n;      // u^n (own cell only)
+    double *w_out;          // u^(i) (may alias w_n on the last stage); or dw/dt if rhs_only
+    const double *scal;     // device scalars: [0] = dt
+    unsigned long long *maxbits;  // [0] = bits of max c_s, [1] = bits of max |v| (non-negative doubles)
+    int *flag;              // set to 1 on rho <= 0 or p <= 0
+    double *sens_prev;      // [0..N) S^K, [N..2N) G^K of the previous step (AV only)
+    double *sens_new;       // same, written on stage 1, committed to sens_prev on the last stage
+    int ncells, nx, ny, nz;
+    double h, gamma, nu, chi;
+    double f_v, f_tau, f_w, s_onset, alpha_max;
+    double rk_a, rk_b, rk_c;  // u^(i) = rk_a u^n + rk_b u^(i-1) + rk_c dt L(u^(i-1))
+    int do_sensor, do_wavespeed, commit_sensor, rhs_only;
+};

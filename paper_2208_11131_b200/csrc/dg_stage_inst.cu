@@ -1,0 +1,69 @@
+// One translation unit per (DG_DIM, DG_M): instantiates the stage kernel for the four physics variants
+// (Euler, NS, AV, NS+AV) and exports plain launch functions for dg_api.cu.  Compiled 16 times by build.py
+// with -DDG_DIM=2|3 -DDG_M=1..8 (keeps ptxas work parallel and each image small).
+#include "dg_stage.cuh"
+#include "dg_dispatch.h"
+
+#ifndef DG_DIM
+#error "compile with -DDG_DIM=2|3 -DDG_M=1..8"
+#endif
+
+namespace {
+
+// opt in to > 48 KB of dynamic shared memory (once per device context, outside any stream capture)
+template <bool VISC, bool AV>
+cudaError_t configure() {
+    using K = dgk::Cfg<DG_DIM, DG_M, VISC, AV>;
+    cudaError_t e = cudaFuncSetAttribute(dgk::dg_stage_kernel<DG_DIM, DG_M, VISC, AV>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, K::kSmemBytes);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(dgk::dg_wavespeed_kernel<DG_DIM, DG_M, VISC, AV>,
+                                cudaFuncAttributeMaxDynamicSharedMemorySize, K::kSmemBytes);
+}
+
+template <bool VISC, bool AV>
+cudaError_t launch(const DgStageArgs &a, cudaStream_t st, int wavespeed_only) {
+    using K = dgk::Cfg<DG_DIM, DG_M, VISC, AV>;
+    const int blocks = (a.ncells + K::C - 1) / K::C;
+    if (wavespeed_only)
+        dgk::dg_wavespeed_kernel<DG_DIM, DG_M, VISC, AV><<<blocks, K::NT, K::kSmemBytes, st>>>(a);
+    else
+        dgk::dg_stage_kernel<DG_DIM, DG_M, VISC, AV><<<blocks, K::NT, K::kSmemBytes, st>>>(a);
+    return cudaGetLastError();
+}
+
+template <bool VISC, bool AV>
+void info(int *c, int *nt, int *smem) {
+    using K = dgk::Cfg<DG_DIM, DG_M, VISC, AV>;
+    *c = K::C;
+    *nt = K::NT;
+    *smem = K::kSmemBytes;
+}
+
+}  // namespace
+
+cudaError_t DG_FN(dg_launch, DG_DIM, DG_M)(int visc, int av, const DgStageArgs *a, cudaStream_t st,
+                                           int wavespeed_only) {
+    if (visc && av) return launch<true, true>(*a, st, wavespeed_only);
+    if (visc) return launch<true, false>(*a, st, wavespeed_only);
+    if (av) return launch<false, true>(*a, st, wavespeed_only);
+    return launch<false, false>(*a, st, wavespeed_only);
+}
+
+cudaError_t DG_FN(dg_upload, DG_DIM, DG_M)(const DgTables *t) {
+    return cudaMemcpyToSymbol(c_tab, t, sizeof(DgTables));
+}
+
+void DG_FN(dg_info, DG_DIM, DG_M)(int visc, int av, int *c, int *nt, int *smem) {
+    if (visc && av) return info<true, true>(c, nt, smem);
+    if (visc) return info<true, false>(c, nt, smem);
+    if (av) return info<false, true>(c, nt, smem);
+    return info<false, false>(c, nt, smem);
+}
+
+cudaError_t DG_FN(dg_config, DG_DIM, DG_M)(int visc, int av) {
+    if (visc && av) return configure<true, true>();
+    if (visc) return configure<true, false>();
+    if (av) return configure<false, true>();
+    return configure<false, false>();
+}

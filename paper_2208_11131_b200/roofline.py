@@ -1,0 +1,80 @@
+"""Algorithmic work model of one RK stage: bytes and flops per cell that any
+implementation of the sum-factorised operator must move / execute.  Holds counts only, no solver arithmetic.
+
+Bytes: each stage reads its input state once and writes its output once; stages 2 and 3 also read u^n
+(SURVEY.md 8(d)):  8 B * V * M * (2 + 3 + 3)/3 per cell per stage.  Halo re-reads are not algorithmic.
+
+Flops (fp64; FMA = 2, divide = sqrt = 1): every 1D matrix application costs 2m per output value; every face
+is counted ONCE (d faces per cell) although the gather kernel evaluates each face from both sides.
+"""
+from __future__ import annotations
+
+NOMINAL_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz = 37.2
+NOMINAL_HBM_GBS = 7700.0
+
+
+def pointwise_flops(d: int, visc: bool, av: bool):
+    """(volume point, face point) flop counts of the point-wise physics, counted from dg_stage.cuh."""
+    prim = 1 + d + 2 * d + 4                      # 1/rho, v, v^2, p
+    euler = d * (d + 1 + 2)                       # d flux columns: d momentum rows (+p), energy row
+    vol = prim + euler
+    hllc = 2 * prim + 6 + 6 + 4 + 8 + (d + 3) + 2 + 3 * (d + 2) + 8
+    face = hllc
+    if visc or av:
+        dv = 3 * d * d + d                        # velocity gradient + divergence
+        vol += dv
+        face += prim + dv
+    if visc:
+        col = 5 * d + 2 * d + 2 * d + 6 + 5       # Pi row, v.Pi, v.dv, d u_th, energy row
+        vol += d * col
+        face += col
+    if av:
+        vol += 3 + 4 + 8 + 2 * d * (d + 2)        # c_s, eps, alpha source, eps * grad u
+        face += 3 + 4 + 2 * (d + 2)
+    return vol, face
+
+
+def stage_flops_per_cell(d: int, m: int, visc: bool, av: bool) -> float:
+    Vc = d + 2
+    V = Vc + (1 if av else 0)
+    grad = visc or av
+    Np, Nf = m ** d, m ** (d - 1)
+    s = 2.0 * m                                   # flops per output value of a 1D sweep
+    fl = V * d * Np * s                           # expansion (Eq. 21)
+    fl += Vc * d * Np * s                         # weak-form derivative, N = sum_a S_a G_a
+    fl += V * d * Np * s                          # projection on the modes
+    if grad:
+        fl += Vc * d * Np * s                     # gradients at the Gauss points
+    # one face per axis per cell
+    per_face = 2 * Vc * Nf * s                    # two one-sided traces
+    nqe = 2 * Vc
+    if grad:
+        per_face += 2 * V * Nf * s + 2 * Vc * Nf * s      # recovery value / normal-gradient partial sums
+        per_face += (d - 1) * Vc * Nf * s                 # transverse gradients
+        nqe = 3 * Vc + V
+    per_face += nqe * (d - 1) * Nf * s            # transverse modal -> nodal
+    per_face += Vc * (d - 1) * Nf * s             # projection of the flux
+    per_face += 2 * Vc * Nf * m * 2               # lift into both cells
+    cv, cf = pointwise_flops(d, visc, av)
+    fl += d * (per_face + Nf * cf) + Np * cv
+    fl += 3 * V * Np                              # stage combine (mean over the stages is ~2.7 fma)
+    return fl
+
+
+def stage_bytes_per_cell(d: int, m: int, av: bool, rk_stages: int = 3) -> float:
+    V = d + 2 + (1 if av else 0)
+    passes = (2 + 3 * (rk_stages - 1)) / rk_stages
+    return 8.0 * V * m ** d * passes
+
+
+def roofline(d, m, visc, av, ncells, t_stage_s, hbm_gbs, fp64_tflops, rk_stages=3):
+    """Both roofs for one stage; `bound` is the one with the larger minimum time."""
+    fl = stage_flops_per_cell(d, m, visc, av) * ncells
+    by = stage_bytes_per_cell(d, m, av, rk_stages) * ncells
+    t_hbm = by / (hbm_gbs * 1e9)
+    t_alu = fl / (fp64_tflops * 1e12)
+    out = dict(flops_per_launch=fl, bytes_per_launch=by, t_hbm_ms=t_hbm * 1e3, t_alu_ms=t_alu * 1e3,
+               hbm_frac=t_hbm / t_stage_s, alu_frac=t_alu / t_stage_s,
+               achieved_gbs=by / t_stage_s / 1e9, achieved_tflops=fl / t_stage_s / 1e12)
+    out["bound"] = "alu" if t_alu >= t_hbm else "hbm"
+    return out

@@ -270,3 +270,24 @@ def random_smooth_modes(dim, ncell, degree, gamma, seed=SEED, amp=0.1, nvar_extr
             w[mode, var] = (0.3 if mode == 0 else 0.05 / (1.0 + deg) ** 2) * np.abs(rng.standard_normal(ncells))
     alpha = np.ascontiguousarray(w[:, Vc, :]).ravel() if nvar_extra else None   # layout [mode*Ncells + cell]
     return np.ascontiguousarray(w[:, :Vc, :]).ravel(), alpha
+
+
+def initial_modes_slabbed(wl: Workload, seed=SEED, layers=8, out=None):
+    """initial_modes() of a large 3D mesh built z-slab by z-slab (bounded host memory); same layout.
+    `out` may be a preallocated flat float64 array (e.g. the numpy view of a pinned torch tensor)."""
+    if wl.dim != 3 or wl.ncell[2] <= layers:
+        w = initial_modes(wl, seed)
+        if out is None:
+            return w
+        out[:] = w
+        return out
+    Vc, M, N = wl.dim + 2, wl.modes, wl.ncells
+    if out is None:
+        out = np.empty(M * Vc * N)
+    full = out.reshape(M * Vc, N)
+    plane = wl.ncell[0] * wl.ncell[1]
+    for z0 in range(0, wl.ncell[2], layers):
+        z1 = min(wl.ncell[2], z0 + layers)
+        part = initial_modes(wl, seed, zslab=(z0, z1)).reshape(M * Vc, (z1 - z0) * plane)
+        full[:, z0 * plane:z1 * plane] = part
+    return out

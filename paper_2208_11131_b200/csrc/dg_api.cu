@@ -112,6 +112,7 @@ struct dg_solver {
     Dispatch fn;
     cudaStream_t stream;
     double *W0, *WA, *WB;
+    double *flux;           // dim * Vc * m^(dim-1) * ncells doubles: projected upper-face fluxes of the current stage
     double *scal;           // [0] dt, [1] t, [2] cmax, [3] vmax, [8..12] totals
     unsigned long long *maxbits;
     int *flag;
@@ -138,6 +139,7 @@ size_t workspace_layout(dg_solver *s, char *base) {
     s->W0 = (double *)take(sb);
     s->WA = (double *)take(sb);
     s->WB = (s->opt.rk_stages >= 3) ? (double *)take(sb) : nullptr;
+    s->flux = (double *)take((size_t)s->dim * s->Vc * (s->M / s->order) * s->ncells * sizeof(double));
     s->scal = (double *)take(16 * sizeof(double));
     s->maxbits = (unsigned long long *)take(2 * sizeof(unsigned long long));
     s->flag = (int *)take(sizeof(int));
@@ -172,6 +174,7 @@ int validate(const dg_mesh *mesh, int order, double gamma, double nu, double chi
 void fill_args(const dg_solver *s, DgStageArgs *a) {
     std::memset(a, 0, sizeof(*a));
     a->scal = s->scal;
+    a->flux = s->flux;
     a->maxbits = s->maxbits;
     a->flag = s->flag;
     a->sens_prev = s->sens_prev;
@@ -410,7 +413,7 @@ int dg_step_async(dg_solver *s, int nsteps) {
         int rc = enqueue_wavespeed(s);
         if (rc) return rc;
     }
-    const int per_step = 1 + s->opt.rk_stages;
+    const int per_step = 1 + 2 * s->opt.rk_stages;   // dt kernel + (face, stage) per RK stage
     if (s->opt.use_graph && nsteps > 0) {
         if (!s->graph) {
             cudaStream_t cap = s->stream;
@@ -512,7 +515,7 @@ int dg_eval_rhs(dg_solver *s, double *out, size_t count, double *alpha_out, size
     a.w_out = s->WA;
     a.rhs_only = 1;
     CU(s->fn.launch(s->visc, s->av, &a, s->stream, 0));
-    s->launches += 1;
+    s->launches += 2;
     int rc = copy_vars(s, out, s->Vc, s->WA, s->V, s->Vc);
     if (rc) return rc;
     if (alpha_out) {

@@ -1,19 +1,21 @@
-// Fused Runge-Kutta-stage kernel of the modal DG operator (sm_100a, fp64 CUDA cores).
+// Runge-Kutta-stage kernels of the modal DG operator (sm_100a, fp64 CUDA cores).
 //
-// One launch = one SSP-RK stage over the whole mesh (Eq. 20-21, 200): every thread block
-// owns C consecutive cells and, for each of them, gathers the cell's own modes and its 2d neighbours'
-// modes, evaluates the surface term of Eq. 20 (face traces, HLLC PAPER.md:106, recovery-based viscous /
-// artificial-viscosity face flux PAPER.md:252-305), the volume term (Eq. 21 expansion by sum factorisation,
-// Euler / Navier-Stokes / AV flux, weak-form derivative, projection), the stage combine and -- on the last
-// stage -- the wave-speed maxima of Eq. 23 for the next step.  dw/dt never touches HBM.
+// One SSP-RK stage (Eq. 20-21, 200) = two launches over the whole mesh:
+//   dg_face_kernel   every cell owns its D upper faces: one-sided traces and recovery partial sums of both
+//                    adjacent cells, HLLC + recovery-based viscous / artificial-viscosity flux
+//                     ONCE per face point, projected on the transverse modes -> `flux`
+//   dg_stage_kernel  lift of the 2D face fluxes, volume term (Eq. 21 expansion by sum factorisation, Euler /
+//                    Navier-Stokes / AV flux, weak-form derivative, projection), shock-sensor bookkeeping, stage
+//                    combine and -- on the last stage -- the wave-speed maxima of Eq. 23 for the next step.
+// dw/dt never touches HBM; the only intermediate in HBM is the projected face flux (D*Vc*m^(D-1) per cell).
 //
 // Shared-memory layout per block (doubles):  [slot][point][cell], cell fastest (C cells), so that a warp
 // whose lanes are consecutive cells reads/writes conflict-free and global accesses coalesce along `cell`
 // (state layout w[(mode*V + var)*Ncells + cell]).
-//   RA   V  x Np   own modes  -> nodal values (in place)
-//   RX   max(D*Vc*Np, 2*NQ*Nf)   face scratch (one axis, both faces)  /  gradients -> fluxes (in place)
-//   ACC  V  x Np   dw/dt in modal space
-// No float atomics, no races: each cell's dw/dt is a fixed-order gather (bit-reproducible run to run).
+//   stage kernel:  RA  V x Np  own modes -> nodal values (in place);  RX  D*Vc*Np  gradients -> fluxes (in place);
+//                  ACC V x Np  dw/dt in modal space
+//   face kernel:   RA  V x Np  own modes;  RX  NQ x Nf  traces / recovered state / gradients of one face
+// No float atomics, no races: each cell's dw/dt is a fixed-order sum (bit-reproducible run to run).
 #pragma once
 
 #include <cuda_runtime.h>
@@ -47,7 +49,7 @@ struct Cfg {
     // face scratch slots per side: uL(Vc) uR(Vc) [u~(V) gn(Vc) gt((D-1) Vc)]
     static constexpr int NQE = GRAD ? (3 * Vc + V) : 2 * Vc;      // slots expanded modal -> nodal
     static constexpr int NQ = NQE + (GRAD ? (D - 1) * Vc : 0);
-    static constexpr int RX = imax(D * Vc * Np, 2 * NQ * Nf);
+    static constexpr int RX = D * Vc * Np;                         // gradients -> fluxes (in place)
     static constexpr int FP = 2 * V * Np + RX;                     // doubles per cell
     static constexpr int NT = 256;
     static constexpr int pick_c() {
@@ -57,7 +59,7 @@ struct Cfg {
     }
     static constexpr int C = pick_c();
     static constexpr int kExtraDoubles = C + 2 * (NT / 32);        // W^K per cell, reduction scratch
-    static constexpr int kSmemBytes = (C * FP + kExtraDoubles) * 8 + 2 * D * C * 4;
+    static constexpr int kSmemBytes = (C * FP + kExtraDoubles) * 8;
     static_assert(kSmemBytes <= kSmemMax, "per-cell footprint exceeds shared memory");
 };
 
@@ -281,94 +283,117 @@ __device__ __forceinline__ void wavespeed_points(const double *RA, double gamma,
 }
 
 // ---------------------------------------------------------------------------------------------------
-// surface term of Eq. 20 for axis A: both faces of every cell of the block (gather form)
+// face kernel: the numerical flux of Eq. 20's surface lines, ONCE per face point.
+// Cell K owns its D "upper" faces (towards +a): left state = K, right state = K_{a+}.  The result, already
+// projected on the transverse modes (sum_k g_k phi_l(xi_k) G^_a), is written to
+//     flux[((A*Vc + v)*Nf + lt) * ncells + cell]
+// and lifted into both adjacent cells by the stage kernel.
 // ---------------------------------------------------------------------------------------------------
-template <int D, int M, bool VISC, bool AV, int A>
-__device__ __forceinline__ void face_axis(const DgStageArgs &p, double *RA, double *RX, double *ACC,
-                                          const int *nbr, int tid) {
+template <int D, int M, bool VISC, bool AV>
+struct FaceCfg {
     using K = Cfg<D, M, VISC, AV>;
-    constexpr int C = K::C, NT = K::NT, V = K::V, Vc = K::Vc, Np = K::Np, Nf = K::Nf, NQ = K::NQ;
+    static constexpr int NT = 256;
+    static constexpr int FP = K::V * K::Np + K::NQ * K::Nf;       // doubles per cell: own modes + one face
+    static constexpr int pick_c() {
+        int c = 32;
+        while (c > 1 && c * FP * 8 > 72 * 1024) c >>= 1;          // three resident blocks per SM
+        return c;
+    }
+    static constexpr int C = pick_c();
+    static constexpr int kSmemBytes = C * FP * 8 + D * C * 4;
+    static_assert(kSmemBytes <= kSmemMax, "face kernel: per-cell footprint exceeds shared memory");
+};
+
+template <int D, int M, bool VISC, bool AV, int A>
+__device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA, double *RX, const int *nbr,
+                                          int cell0, int tid) {
+    using K = Cfg<D, M, VISC, AV>;
+    using FK = FaceCfg<D, M, VISC, AV>;
+    constexpr int C = FK::C, NT = FK::NT, V = K::V, Vc = K::Vc, Np = K::Np, Nf = K::Nf;
     constexpr bool GRAD = K::GRAD;
     constexpr int SA = ipow(M, A);               // stride of axis A inside the cell
-    constexpr int SIDE = NQ * Nf * C;            // doubles per face side in RX
     constexpr int oUL = 0, oUR = Vc, oUT = 2 * Vc, oGN = 2 * Vc + V, oGT = 3 * Vc + V;
     const double ih = 1.0 / p.h;
 
-    // F1: contract the normal axis (PAPER.md:171 traces; 294-299 recovery partial sums)
-    for (int it = tid; it < 2 * V * Nf * C; it += NT) {
-        const int cell = it % C;
-        int r = it / C;
-        const int lt = r % Nf;
-        r /= Nf;
-        const int v = r % V;
-        const int s = r / V;   // 0: face towards -A (neighbour is the LEFT state), 1: face towards +A
-        const int base = pencil_base<M, SA>(lt);
-        const int nc = nbr[(2 * A + s) * C + cell];
-        double own[M], nb[M];
+    // F1: contract the normal axis (PAPER.md:171 traces; 294-299 recovery partial sums).  A thread keeps one
+    // cell (NT % C == 0); all its neighbour loads are issued before the first use.
+    {
+        static_assert(NT % C == 0, "threads per block must be a multiple of cells per block");
+        constexpr int NIT = (V * Nf * C + NT - 1) / NT;
+        const int cell = tid % C;
+        const int nc = nbr[A * C + cell];
+        double nb[NIT][M];
 #pragma unroll
-        for (int l = 0; l < M; ++l) nb[l] = p.w_prev[(size_t)((base + l * SA) * V + v) * p.ncells + nc];
+        for (int k = 0; k < NIT; ++k) {
+            const int r = tid / C + k * (NT / C);          // v*Nf + lt
+            if (r < V * Nf) {
+                const int base = pencil_base<M, SA>(r % Nf);
+                const int v = r / Nf;
 #pragma unroll
-        for (int l = 0; l < M; ++l) own[l] = RA[(v * Np + base + l * SA) * C + cell];
-        double *F = RX + s * SIDE + lt * C + cell;
-        double uL = 0.0, uR = 0.0, ut = 0.0, gn = 0.0;
-#pragma unroll
-        for (int l = 0; l < M; ++l) {
-            const double lf = s ? own[l] : nb[l];
-            const double rt = s ? nb[l] : own[l];
-            uL = fma(c_tab.Pend[1][l], lf, uL);
-            uR = fma(c_tab.Pend[0][l], rt, uR);
-            if (GRAD) {
-                ut = fma(c_tab.Rv[0][l], lf, ut);
-                ut = fma(c_tab.Rv[1][l], rt, ut);
-                gn = fma(c_tab.Gv[0][l], lf, gn);
-                gn = fma(c_tab.Gv[1][l], rt, gn);
+                for (int l = 0; l < M; ++l)
+                    nb[k][l] = __ldg(p.w_prev + (size_t)((base + l * SA) * V + v) * p.ncells + nc);
             }
         }
-        if (v < Vc) {
-            F[(oUL + v) * Nf * C] = uL;
-            F[(oUR + v) * Nf * C] = uR;
-            if (GRAD) F[(oGN + v) * Nf * C] = gn * ih;
+#pragma unroll
+        for (int k = 0; k < NIT; ++k) {
+            const int r = tid / C + k * (NT / C);
+            if (r < V * Nf) {
+                const int lt = r % Nf;
+                const int v = r / Nf;
+                const int base = pencil_base<M, SA>(lt);
+                double own[M];
+#pragma unroll
+                for (int l = 0; l < M; ++l) own[l] = RA[(v * Np + base + l * SA) * C + cell];
+                double *F = RX + lt * C + cell;
+                double uL = 0.0, uR = 0.0, ut = 0.0, gn = 0.0;
+#pragma unroll
+                for (int l = 0; l < M; ++l) {
+                    uL = fma(c_tab.Pend[1][l], own[l], uL);
+                    uR = fma(c_tab.Pend[0][l], nb[k][l], uR);
+                    if (GRAD) {
+                        ut = fma(c_tab.Rv[0][l], own[l], ut);
+                        ut = fma(c_tab.Rv[1][l], nb[k][l], ut);
+                        gn = fma(c_tab.Gv[0][l], own[l], gn);
+                        gn = fma(c_tab.Gv[1][l], nb[k][l], gn);
+                    }
+                }
+                if (v < Vc) {
+                    F[(oUL + v) * Nf * C] = uL;
+                    F[(oUR + v) * Nf * C] = uR;
+                    if (GRAD) F[(oGN + v) * Nf * C] = gn * ih;
+                }
+                if (GRAD) F[(oUT + v) * Nf * C] = ut;
+            }
         }
-        if (GRAD) F[(oUT + v) * Nf * C] = ut;
     }
     __syncthreads();
 
     // F2: transverse modal -> nodal on the face (cell basis kept transversally)
     if (M > 1) {
-#pragma unroll
-        for (int s = 0; s < 2; ++s)
-            sweep<DG_SEL_V, M, Nf, 1, C, NT, 1, false, false>(RX + s * SIDE, 0, RX + s * SIDE, K::NQE, 1.0, tid);
+        sweep<DG_SEL_V, M, Nf, 1, C, NT, 1, false, false>(RX, 0, RX, K::NQE, 1.0, tid);
         __syncthreads();
         if (D == 3) {
-#pragma unroll
-            for (int s = 0; s < 2; ++s)
-                sweep<DG_SEL_V, M, Nf, M, C, NT, 1, false, false>(RX + s * SIDE, 0, RX + s * SIDE, K::NQE, 1.0, tid);
+            sweep<DG_SEL_V, M, Nf, M, C, NT, 1, false, false>(RX, 0, RX, K::NQE, 1.0, tid);
             __syncthreads();
         }
     }
     if (GRAD) {
         // transverse derivatives of the recovered face polynomial
-#pragma unroll
-        for (int s = 0; s < 2; ++s) {
-            sweep<DG_SEL_DHAT, M, Nf, 1, C, NT, 1, false, true>(RX + s * SIDE + oUT * Nf * C, 0,
-                                                               RX + s * SIDE + oGT * Nf * C, Vc, 2.0 * ih, tid);
-            if (D == 3)
-                sweep<DG_SEL_DHAT, M, Nf, M, C, NT, 1, false, true>(RX + s * SIDE + oUT * Nf * C, 0,
-                                                                   RX + s * SIDE + (oGT + Vc) * Nf * C, Vc,
-                                                                   2.0 * ih, tid);
-        }
+        sweep<DG_SEL_DHAT, M, Nf, 1, C, NT, 1, false, true>(RX + oUT * Nf * C, 0, RX + oGT * Nf * C, Vc, 2.0 * ih,
+                                                           tid);
+        if (D == 3)
+            sweep<DG_SEL_DHAT, M, Nf, M, C, NT, 1, false, true>(RX + oUT * Nf * C, 0, RX + (oGT + Vc) * Nf * C, Vc,
+                                                               2.0 * ih, tid);
         __syncthreads();
     }
 
     // F3: numerical flux at every face point; result overwrites the uL slots
     {
         bool bad = false;
-        for (int it = tid; it < 2 * Nf * C; it += NT) {
+        for (int it = tid; it < Nf * C; it += NT) {
             const int cell = it % C;
-            const int r = it / C;
-            const int k = r % Nf;
-            const int s = r / Nf;
-            double *F = RX + s * SIDE + k * C + cell;
+            const int k = it / C;
+            double *F = RX + k * C + cell;
             double uL[Vc], uR[Vc], Fh[Vc];
 #pragma unroll
             for (int v = 0; v < Vc; ++v) {
@@ -416,44 +441,76 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, double *RA, doub
     __syncthreads();
 
     // F4: project the face flux on the transverse modes (g_k phi_l(xi_k) of Eq. 20's surface lines)
-    if (M > 1) {
-#pragma unroll
-        for (int s = 0; s < 2; ++s)
-            sweep<DG_SEL_VTG, M, Nf, 1, C, NT, 1, false, false>(RX + s * SIDE, 0, RX + s * SIDE, Vc, 1.0, tid);
-        __syncthreads();
-        if (D == 3) {
-#pragma unroll
-            for (int s = 0; s < 2; ++s)
-                sweep<DG_SEL_VTG, M, Nf, M, C, NT, 1, false, false>(RX + s * SIDE, 0, RX + s * SIDE, Vc, 1.0, tid);
-            __syncthreads();
-        }
-    } else {
-        // single point: weight g_0^(D-1) = 2^(D-1)
-        for (int it = tid; it < 2 * Vc * C; it += NT) {
-            const int cell = it % C;
-            const int r = it / C;
-            RX[(r / Vc) * SIDE + (r % Vc) * Nf * C + cell] *= (D == 3 ? 4.0 : 2.0);
-        }
+    if (M > 1 && D == 3) {
+        sweep<DG_SEL_VTG, M, Nf, 1, C, NT, 1, false, false>(RX, 0, RX, Vc, 1.0, tid);
         __syncthreads();
     }
-
-    // F5: lift along the normal: dw_l -= pref [P_l(+1) F^(+) - P_l(-1) F^(-)]   (Eq. 20, readings A3/A4)
+    // last projection sweep (or the single-point weight g_0^(D-1) = 2^(D-1)) straight to global memory
     {
-        const double pref = (D == 3 ? 0.25 : 0.5) * ih;
-        for (int it = tid; it < Vc * Nf * C; it += NT) {
+        constexpr int STR = (D == 3) ? M : 1;
+        constexpr int NPEN = Nf / M;
+        double *out = p.flux + (size_t)A * Vc * Nf * p.ncells;
+        for (int it = tid; it < Vc * NPEN * C; it += NT) {
             const int cell = it % C;
             const int r = it / C;
-            const int lt = r % Nf;
-            const int v = r / Nf;
-            const double Fm = RX[(v * Nf + lt) * C + cell];          // face towards -A
-            const double Fp = RX[SIDE + (v * Nf + lt) * C + cell];   // face towards +A
-            const int base = pencil_base<M, SA>(lt);
+            const int pen = r % NPEN;
+            const int v = r / NPEN;
+            if (cell0 + cell >= p.ncells) continue;
+            const int off = v * Nf + pencil_base<M, STR>(pen);
+            double in[M];
 #pragma unroll
-            for (int l = 0; l < M; ++l)
-                ACC[(v * Np + base + l * SA) * C + cell] += pref * (c_tab.Pend[0][l] * Fm - c_tab.Pend[1][l] * Fp);
+            for (int i = 0; i < M; ++i) in[i] = RX[(off + i * STR) * C + cell];
+#pragma unroll
+            for (int j = 0; j < M; ++j) {
+                double acc;
+                if (M > 1) {
+                    acc = c_tab.VtG[j * 8] * in[0];
+#pragma unroll
+                    for (int i = 1; i < M; ++i) acc = fma(c_tab.VtG[j * 8 + i], in[i], acc);
+                } else {
+                    acc = in[0] * (D == 3 ? 4.0 : 2.0);
+                }
+                out[(size_t)(off + j * STR) * p.ncells + cell0 + cell] = acc;
+            }
         }
     }
     __syncthreads();
+}
+
+template <int D, int M, bool VISC, bool AV>
+__global__ void __launch_bounds__(256, 3) dg_face_kernel(const DgStageArgs p) {
+    using K = Cfg<D, M, VISC, AV>;
+    using FK = FaceCfg<D, M, VISC, AV>;
+    constexpr int C = FK::C, NT = FK::NT, V = K::V, Np = K::Np;
+    extern __shared__ double smem[];
+    double *RA = smem;
+    double *RX = RA + V * Np * C;
+    int *nbr = reinterpret_cast<int *>(RX + K::NQ * K::Nf * C);
+    const int tid = threadIdx.x;
+    const int cell0 = blockIdx.x * C;
+    if (tid < C) {
+        const int c = min(cell0 + tid, p.ncells - 1);
+        const int ix = c % p.nx;
+        const int iy = (c / p.nx) % p.ny;
+        const int iz = c / (p.nx * p.ny);
+        nbr[0 * C + tid] = c + ((ix == p.nx - 1) ? 1 - p.nx : 1);
+        nbr[1 * C + tid] = c + ((iy == p.ny - 1) ? -(p.ny - 1) * p.nx : p.nx);
+        if (D == 3) {
+            const int pl = p.nx * p.ny;
+            nbr[(D - 1) * C + tid] = c + ((iz == p.nz - 1) ? -(p.nz - 1) * pl : pl);
+        }
+    }
+    for (int it = tid; it < V * Np * C; it += NT) {
+        const int cell = it % C;
+        const int r = it / C;              // global slot order: mode*V + v
+        const int mode = r / V, v = r % V;
+        const int cg = min(cell0 + cell, p.ncells - 1);
+        RA[(v * Np + mode) * C + cell] = p.w_prev[(size_t)r * p.ncells + cg];
+    }
+    __syncthreads();
+    face_axis<D, M, VISC, AV, 0>(p, RA, RX, nbr, cell0, tid);
+    face_axis<D, M, VISC, AV, 1>(p, RA, RX, nbr, cell0, tid);
+    if (D == 3) face_axis<D, M, VISC, AV, (D == 3 ? 2 : 0)>(p, RA, RX, nbr, cell0, tid);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -470,46 +527,81 @@ __global__ void __launch_bounds__(256, 2) dg_stage_kernel(const DgStageArgs p) {
     double *ACC = RX + K::RX * C;
     double *Wk = ACC + V * Np * C;
     double *red = Wk + C;
-    int *nbr = reinterpret_cast<int *>(red + 2 * (NT / 32));
     const int tid = threadIdx.x;
     const int cell0 = blockIdx.x * C;
 
-    if (tid < C) {
-        const int c = min(cell0 + tid, p.ncells - 1);
-        const int ix = c % p.nx;
-        const int iy = (c / p.nx) % p.ny;
-        const int iz = c / (p.nx * p.ny);
-        nbr[0 * C + tid] = c + ((ix == 0) ? p.nx - 1 : -1);
-        nbr[1 * C + tid] = c + ((ix == p.nx - 1) ? 1 - p.nx : 1);
-        nbr[2 * C + tid] = c + ((iy == 0) ? (p.ny - 1) * p.nx : -p.nx);
-        nbr[3 * C + tid] = c + ((iy == p.ny - 1) ? -(p.ny - 1) * p.nx : p.nx);
-        if (D == 3) {
-            const int pl = p.nx * p.ny;
-            nbr[(2 * (D - 1)) * C + tid] = c + ((iz == 0) ? (p.nz - 1) * pl : -pl);
-            nbr[(2 * (D - 1) + 1) * C + tid] = c + ((iz == p.nz - 1) ? -(p.nz - 1) * pl : pl);
-        }
-        if (AV) {
-            // wiggle source of Eq. 45 from the previous step's sensor (readings A14, A15)
-            const double S = p.sens_prev[c];
-            const double G = p.sens_prev[p.ncells + c];
-            Wk[tid] = (S > p.s_onset) ? p.f_w * fmax(0.0, G) : 0.0;
+    // every thread works on one fixed cell of the block (NT is a multiple of C)
+    static_assert(NT % C == 0, "threads per block must be a multiple of cells per block");
+    const int cl = tid % C;
+    const int cg = min(cell0 + cl, p.ncells - 1);
+    int nbm[D];                                  // lower neighbour along each axis (periodic wrap)
+    {
+        const int ix = cg % p.nx;
+        const int iy = (cg / p.nx) % p.ny;
+        const int iz = cg / (p.nx * p.ny);
+        nbm[0] = cg + ((ix == 0) ? p.nx - 1 : -1);
+        nbm[1] = cg + ((iy == 0) ? (p.ny - 1) * p.nx : -p.nx);
+        if (D == 3) nbm[D - 1] = cg + ((iz == 0) ? (p.nz - 1) * p.nx * p.ny : -p.nx * p.ny);
+    }
+    // ---- front loads, all in flight before the first barrier: face fluxes of the 2D faces, own modes ----
+    constexpr int NFL = Vc * K::Nf;                       // flux values per cell and axis
+    constexpr int NLIFT = (NFL * C + NT - 1) / NT;
+    double Fp[D][NLIFT], Fm[D][NLIFT];
+#pragma unroll
+    for (int a = 0; a < D; ++a) {
+        const double *fl = p.flux + (size_t)a * NFL * p.ncells;
+#pragma unroll
+        for (int k = 0; k < NLIFT; ++k) {
+            const int r = tid / C + k * (NT / C);
+            if (r < NFL) {
+                Fp[a][k] = __ldg(fl + (size_t)r * p.ncells + cg);
+                Fm[a][k] = __ldg(fl + (size_t)r * p.ncells + nbm[a]);
+            }
         }
     }
+    if (!p.rhs_only && cl % 4 == 0) {
+        // u^n is needed only by the stage combine at the very end: start it towards L2 now
+        for (int r = tid / C; r < V * Np; r += NT / C)
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(p.w_n + (size_t)r * p.ncells + cg));
+    }
+    if (AV && tid < C) {
+        // wiggle source of Eq. 45 from the previous step's sensor (readings A14, A15)
+        const double S = p.sens_prev[cg];
+        const double G = p.sens_prev[p.ncells + cg];
+        Wk[tid] = (S > p.s_onset) ? p.f_w * fmax(0.0, G) : 0.0;
+    }
     // own modes -> RA, zero ACC
-    for (int it = tid; it < V * Np * C; it += NT) {
-        const int cell = it % C;
-        const int r = it / C;              // global slot order: mode*V + v
+    for (int r = tid / C; r < V * Np; r += NT / C) {      // global slot order: r = mode*V + v
         const int mode = r / V, v = r % V;
-        const int cg = min(cell0 + cell, p.ncells - 1);
-        RA[(v * Np + mode) * C + cell] = p.w_prev[(size_t)r * p.ncells + cg];
-        ACC[it] = 0.0;
+        RA[(v * Np + mode) * C + cl] = p.w_prev[(size_t)r * p.ncells + cg];
+        ACC[r * C + cl] = 0.0;
     }
     __syncthreads();
 
-    // ---- surface term ----
-    face_axis<D, M, VISC, AV, 0>(p, RA, RX, ACC, nbr, tid);
-    face_axis<D, M, VISC, AV, 1>(p, RA, RX, ACC, nbr, tid);
-    if (D == 3) face_axis<D, M, VISC, AV, (D == 3 ? 2 : 0)>(p, RA, RX, ACC, nbr, tid);
+    // ---- surface term: lift the face fluxes of dg_face_kernel along each normal (Eq. 20, readings A3/A4) ----
+    //      dw_l -= pref [P_l(+1) F^(a+) - P_l(-1) F^(a-)],  F^(a+) = this cell's upper face, F^(a-) = the lower
+    //      neighbour's upper face; every (variable, transverse mode) item owns one modal pencil along the axis
+    {
+        const double pref = (D == 3 ? 0.25 : 0.5) / p.h;
+#pragma unroll
+        for (int a = 0; a < D; ++a) {
+            const int SA = (a == 0) ? 1 : (a == 1 ? M : M * M);
+#pragma unroll
+            for (int k = 0; k < NLIFT; ++k) {
+                const int r = tid / C + k * (NT / C);     // v*Nf + lt
+                if (r < NFL) {
+                    const int lt = r % K::Nf;
+                    const int v = r / K::Nf;
+                    const int base = (lt / SA) * (SA * M) + (lt % SA);
+#pragma unroll
+                    for (int l = 0; l < M; ++l)
+                        ACC[(v * Np + base + l * SA) * C + cl] +=
+                            pref * (c_tab.Pend[0][l] * Fm[a][k] - c_tab.Pend[1][l] * Fp[a][k]);
+                }
+            }
+            __syncthreads();
+        }
+    }
 
     // ---- volume term ----
     expand_volume<D, M, C, NT>(RA, V, tid);                       // V1: Eq. 21

@@ -5,6 +5,7 @@ struct DgStageArgs {
     const double *w_prev;   // stage input u^(i-1): halo + own reads
     const double *w_n;      // u^n (own cell only)
     double *w_out;          // u^(i) (may alias w_n on the last stage); or dw/dt if rhs_only
+    double *flux;           // projected upper-face fluxes [axis][var][transverse mode][cell] (face kernel -> stage kernel)
     const double *scal;     // device scalars: [0] = dt
     unsigned long long *maxbits;  // [0] = bits of max c_s, [1] = bits of max |v| (non-negative doubles)
     int *flag;              // set to 1 on rho <= 0 or p <= 0

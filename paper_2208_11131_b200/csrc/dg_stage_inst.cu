@@ -1,4 +1,4 @@
-// One translation unit per (DG_DIM, DG_M): instantiates the stage kernel for the four physics variants
+// One translation unit per (DG_DIM, DG_M): instantiates the face + stage kernels for the four physics variants
 // (Euler, NS, AV, NS+AV) and exports plain launch functions for dg_api.cu.  Compiled 16 times by build.py
 // with -DDG_DIM=2|3 -DDG_M=1..8 (keeps ptxas work parallel and each image small).
 #include "dg_stage.cuh"
@@ -17,6 +17,9 @@ cudaError_t configure() {
     cudaError_t e = cudaFuncSetAttribute(dgk::dg_stage_kernel<DG_DIM, DG_M, VISC, AV>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, K::kSmemBytes);
     if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(dgk::dg_face_kernel<DG_DIM, DG_M, VISC, AV>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             dgk::FaceCfg<DG_DIM, DG_M, VISC, AV>::kSmemBytes);
+    if (e != cudaSuccess) return e;
     return cudaFuncSetAttribute(dgk::dg_wavespeed_kernel<DG_DIM, DG_M, VISC, AV>,
                                 cudaFuncAttributeMaxDynamicSharedMemorySize, K::kSmemBytes);
 }
@@ -25,10 +28,16 @@ template <bool VISC, bool AV>
 cudaError_t launch(const DgStageArgs &a, cudaStream_t st, int wavespeed_only) {
     using K = dgk::Cfg<DG_DIM, DG_M, VISC, AV>;
     const int blocks = (a.ncells + K::C - 1) / K::C;
-    if (wavespeed_only)
+    if (wavespeed_only) {
         dgk::dg_wavespeed_kernel<DG_DIM, DG_M, VISC, AV><<<blocks, K::NT, K::kSmemBytes, st>>>(a);
-    else
+    } else {
+        using FK = dgk::FaceCfg<DG_DIM, DG_M, VISC, AV>;
+        const int fblocks = (a.ncells + FK::C - 1) / FK::C;
+        dgk::dg_face_kernel<DG_DIM, DG_M, VISC, AV><<<fblocks, FK::NT, FK::kSmemBytes, st>>>(a);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
         dgk::dg_stage_kernel<DG_DIM, DG_M, VISC, AV><<<blocks, K::NT, K::kSmemBytes, st>>>(a);
+    }
     return cudaGetLastError();
 }
 

@@ -36,7 +36,13 @@ namespace dgk {
 __host__ __device__ constexpr int ipow(int b, int e) { return e <= 0 ? 1 : b * ipow(b, e - 1); }
 __host__ __device__ constexpr int imax(int a, int b) { return a > b ? a : b; }
 
-constexpr int kSmemBudget = 112 * 1024;   // two resident blocks per SM (228 KB, 1 KB reserved per block)
+#ifndef DG_STAGE_NT
+#define DG_STAGE_NT 256
+#endif
+#ifndef DG_STAGE_MINB
+#define DG_STAGE_MINB 2
+#endif
+constexpr int kSmemBudget = (227 * 1024) / DG_STAGE_MINB - 1024;   // DG_STAGE_MINB resident blocks per SM
 constexpr int kSmemMax = 227 * 1024;
 
 template <int D, int M, bool VISC, bool AV>
@@ -51,7 +57,7 @@ struct Cfg {
     static constexpr int NQ = NQE + (GRAD ? (D - 1) * Vc : 0);
     static constexpr int RX = D * Vc * Np;                         // gradients -> fluxes (in place)
     static constexpr int FP = 2 * V * Np + RX;                     // doubles per cell
-    static constexpr int NT = 256;
+    static constexpr int NT = DG_STAGE_NT;
     static constexpr int pick_c() {
         int c = 32;
         while (c > 1 && c * FP * 8 > kSmemBudget) c >>= 1;
@@ -282,6 +288,29 @@ __device__ __forceinline__ void wavespeed_points(const double *RA, double gamma,
     block_max2<NT>(cmax, vmax, red, maxbits, tid);
 }
 
+// Own modes of the block's cells, global [r = mode*V + v][cell] -> shared [v][mode][cell].  Thread `tid` keeps
+// cell tid % C; its loads are issued in batches of up to 12 before the first store (one DRAM round trip per batch).
+template <int V, int Np, int C, int NT>
+__device__ __forceinline__ void load_own_modes(const double *__restrict__ w, int ncells, int cg, double *RA, int tid) {
+    constexpr int NR = (V * Np * C + NT - 1) / NT;
+    constexpr int RB = NR < 12 ? NR : 12;
+    const int cl = tid % C;
+#pragma unroll
+    for (int k0 = 0; k0 < NR; k0 += RB) {
+        double t[RB];
+#pragma unroll
+        for (int j = 0; j < RB; ++j) {
+            const int r = tid / C + (k0 + j) * (NT / C);
+            if (k0 + j < NR && r < V * Np) t[j] = __ldg(w + (size_t)r * ncells + cg);
+        }
+#pragma unroll
+        for (int j = 0; j < RB; ++j) {
+            const int r = tid / C + (k0 + j) * (NT / C);
+            if (k0 + j < NR && r < V * Np) RA[((r % V) * Np + r / V) * C + cl] = t[j];
+        }
+    }
+}
+
 // ---------------------------------------------------------------------------------------------------
 // face kernel: the numerical flux of Eq. 20's surface lines, ONCE per face point.
 // Cell K owns its D "upper" faces (towards +a): left state = K, right state = K_{a+}.  The result, already
@@ -500,13 +529,7 @@ __global__ void __launch_bounds__(256, 3) dg_face_kernel(const DgStageArgs p) {
             nbr[(D - 1) * C + tid] = c + ((iz == p.nz - 1) ? -(p.nz - 1) * pl : pl);
         }
     }
-    for (int it = tid; it < V * Np * C; it += NT) {
-        const int cell = it % C;
-        const int r = it / C;              // global slot order: mode*V + v
-        const int mode = r / V, v = r % V;
-        const int cg = min(cell0 + cell, p.ncells - 1);
-        RA[(v * Np + mode) * C + cell] = p.w_prev[(size_t)r * p.ncells + cg];
-    }
+    load_own_modes<V, Np, C, NT>(p.w_prev, p.ncells, min(cell0 + tid % C, p.ncells - 1), RA, tid);
     __syncthreads();
     face_axis<D, M, VISC, AV, 0>(p, RA, RX, nbr, cell0, tid);
     face_axis<D, M, VISC, AV, 1>(p, RA, RX, nbr, cell0, tid);
@@ -517,7 +540,7 @@ __global__ void __launch_bounds__(256, 3) dg_face_kernel(const DgStageArgs p) {
 // the stage kernel
 // ---------------------------------------------------------------------------------------------------
 template <int D, int M, bool VISC, bool AV>
-__global__ void __launch_bounds__(256, 2) dg_stage_kernel(const DgStageArgs p) {
+__global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(const DgStageArgs p) {
     using K = Cfg<D, M, VISC, AV>;
     constexpr int C = K::C, NT = K::NT, V = K::V, Vc = K::Vc, Np = K::Np;
     constexpr bool GRAD = K::GRAD;
@@ -571,11 +594,8 @@ __global__ void __launch_bounds__(256, 2) dg_stage_kernel(const DgStageArgs p) {
         Wk[tid] = (S > p.s_onset) ? p.f_w * fmax(0.0, G) : 0.0;
     }
     // own modes -> RA, zero ACC
-    for (int r = tid / C; r < V * Np; r += NT / C) {      // global slot order: r = mode*V + v
-        const int mode = r / V, v = r % V;
-        RA[(v * Np + mode) * C + cl] = p.w_prev[(size_t)r * p.ncells + cg];
-        ACC[r * C + cl] = 0.0;
-    }
+    load_own_modes<V, Np, C, NT>(p.w_prev, p.ncells, cg, RA, tid);   // global slot order: r = mode*V + v
+    for (int r = tid / C; r < V * Np; r += NT / C) ACC[r * C + cl] = 0.0;
     __syncthreads();
 
     // ---- surface term: lift the face fluxes of dg_face_kernel along each normal (Eq. 20, readings A3/A4) ----
@@ -716,24 +736,36 @@ __global__ void __launch_bounds__(256, 2) dg_stage_kernel(const DgStageArgs p) {
 
     // ---- stage combine ----
     const double cdt = p.rhs_only ? 1.0 : p.rk_c * p.scal[0];
-    for (int it = tid; it < V * Np * C; it += NT) {
-        const int cell = it % C;
-        const int r = it / C;
-        const int mode = r / V, v = r % V;
-        const int cg = cell0 + cell;
-        const bool active = cg < p.ncells;
-        const size_t gi = (size_t)r * p.ncells + (active ? cg : p.ncells - 1);
-        const double L = ACC[(v * Np + mode) * C + cell];
-        double wnew;
-        if (p.rhs_only) {
-            wnew = L;
-        } else {
-            wnew = p.rk_a * p.w_n[gi];
-            if (p.rk_b != 0.0) wnew = fma(p.rk_b, p.w_prev[gi], wnew);
-            wnew = fma(cdt, L, wnew);
+    {
+        constexpr int NR = (V * Np * C + NT - 1) / NT;
+        constexpr int RB = NR < 6 ? NR : 6;
+        const bool active = cell0 + cl < p.ncells;
+        const bool need_n = !p.rhs_only, need_p = !p.rhs_only && p.rk_b != 0.0;
+#pragma unroll
+        for (int k0 = 0; k0 < NR; k0 += RB) {
+            double wn[RB], wp[RB];
+#pragma unroll
+            for (int j = 0; j < RB; ++j) {
+                const int r = tid / C + (k0 + j) * (NT / C);
+                wn[j] = wp[j] = 0.0;
+                if (k0 + j < NR && r < V * Np) {
+                    if (need_n) wn[j] = __ldg(p.w_n + (size_t)r * p.ncells + cg);
+                    if (need_p) wp[j] = __ldg(p.w_prev + (size_t)r * p.ncells + cg);
+                }
+            }
+#pragma unroll
+            for (int j = 0; j < RB; ++j) {
+                const int r = tid / C + (k0 + j) * (NT / C);
+                if (k0 + j < NR && r < V * Np) {
+                    const int mode = r / V, v = r % V;
+                    const double L = ACC[(v * Np + mode) * C + cl];
+                    double wnew = L;
+                    if (!p.rhs_only) wnew = fma(cdt, L, fma(p.rk_b, wp[j], p.rk_a * wn[j]));
+                    if (active) p.w_out[(size_t)r * p.ncells + cg] = wnew;
+                    if (p.do_wavespeed) RA[(v * Np + mode) * C + cl] = wnew;
+                }
+            }
         }
-        if (active) p.w_out[gi] = wnew;
-        if (p.do_wavespeed) RA[(v * Np + mode) * C + cell] = wnew;
     }
     // ---- wave speeds of the new state for the next step's Eq. 23 ----
     if (p.do_wavespeed) {
@@ -745,7 +777,7 @@ __global__ void __launch_bounds__(256, 2) dg_stage_kernel(const DgStageArgs p) {
 
 // standalone wave-speed kernel (after dg_set_state): load -> expand -> max
 template <int D, int M, bool VISC, bool AV>
-__global__ void __launch_bounds__(256, 2) dg_wavespeed_kernel(const DgStageArgs p) {
+__global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_wavespeed_kernel(const DgStageArgs p) {
     using K = Cfg<D, M, VISC, AV>;
     constexpr int C = K::C, NT = K::NT, V = K::V, Vc = K::Vc, Np = K::Np;
     extern __shared__ double smem[];

@@ -29,6 +29,13 @@
 #define DG_SEL_S 2
 #define DG_SEL_VTG 3
 
+#ifndef DG_STAGE_NT
+#define DG_STAGE_NT 256
+#endif
+#ifndef DG_STAGE_MINB
+#define DG_STAGE_MINB 2
+#endif
+
 __constant__ DgTables c_tab;
 
 namespace dgk {
@@ -36,12 +43,6 @@ namespace dgk {
 __host__ __device__ constexpr int ipow(int b, int e) { return e <= 0 ? 1 : b * ipow(b, e - 1); }
 __host__ __device__ constexpr int imax(int a, int b) { return a > b ? a : b; }
 
-#ifndef DG_STAGE_NT
-#define DG_STAGE_NT 256
-#endif
-#ifndef DG_STAGE_MINB
-#define DG_STAGE_MINB 2
-#endif
 constexpr int kSmemBudget = (227 * 1024) / DG_STAGE_MINB - 1024;   // DG_STAGE_MINB resident blocks per SM
 constexpr int kSmemMax = 227 * 1024;
 
@@ -52,7 +53,7 @@ struct Cfg {
     static constexpr int V = Vc + (AV ? 1 : 0);
     static constexpr int Np = ipow(M, D);
     static constexpr int Nf = ipow(M, D - 1);
-    // face scratch slots per side: uL(Vc) uR(Vc) [u~(V) gn(Vc) gt((D-1) Vc)]
+    // face scratch slots: uL(Vc) uR(Vc) [u~(V) gn(Vc) gt((D-1) Vc)]
     static constexpr int NQE = GRAD ? (3 * Vc + V) : 2 * Vc;      // slots expanded modal -> nodal
     static constexpr int NQ = NQE + (GRAD ? (D - 1) * Vc : 0);
     static constexpr int RX = D * Vc * Np;                         // gradients -> fluxes (in place)
@@ -64,10 +65,34 @@ struct Cfg {
         return c;
     }
     static constexpr int C = pick_c();
-    static constexpr int kExtraDoubles = C + 2 * (NT / 32);        // W^K per cell, reduction scratch
+    // W^K per cell, wave-speed reduction scratch, partial sensor sums
+    static constexpr int kExtraDoubles = C + 2 * (NT / 32) + (AV ? 4 * (NT / 32) * C : 0);
     static constexpr int kSmemBytes = (C * FP + kExtraDoubles) * 8;
     static_assert(kSmemBytes <= kSmemMax, "per-cell footprint exceeds shared memory");
+    // A tile of m x m points (the two fastest axes) is swept in registers when it fits (m <= 5).
+    static constexpr bool BLK = (M >= 2) && (M * M <= 25);
 };
+
+// Shared-memory arrays are indexed by a flat point index P = slot*NPTS + p and the cell:  offset = at(P)*C + cell.
+// With C = 8 a row of cells is half a 128-byte bank line, and rows whose P differ by a multiple of 2 collide when
+// the lanes of a warp walk over planes / slots (strides that are multiples of 16 doubles).  For even m the two rows
+// of a pair are exchanged according to the parity of (plane index + slot index), which makes every access pattern
+// of the kernels below conflict-free (pencils along any axis, m x m tiles, point-wise, row-wise I/O).
+template <int PL, int NPTS, bool SWZ>
+struct Lay {
+    static __device__ __forceinline__ int at(int P) {
+        if (SWZ) {
+            const int par = P / PL + (NPTS > PL ? P / NPTS : 0);
+            return P ^ (par & 1);
+        }
+        return P;
+    }
+    // parity of tile g (PL points per tile): rows q and q^1 of the tile are exchanged when it is 1
+    static __device__ __forceinline__ int tile_par(int g) {
+        return SWZ ? ((g + (NPTS > PL ? g / (NPTS / PL) : 0)) & 1) : 0;
+    }
+};
+__host__ __device__ constexpr bool use_swizzle(int M, int C) { return (M % 2 == 0) && (C == 8); }
 
 template <int SEL>
 __device__ __forceinline__ double mat(int idx) {
@@ -83,12 +108,12 @@ __device__ __forceinline__ int pencil_base(int pen) {
     return (pen / STRIDE) * (STRIDE * M) + (pen % STRIDE);
 }
 
-// Apply one 1D matrix along one axis to `nslots` arrays of NPTS points:
-//   dst[slot][p] (+)= scale * sum_i MAT[j][i] * (sum_{k<NSUM} src[k*sum_stride + slot][p_i])
+// Apply one 1D matrix along one axis to `nslots` arrays of NPTS points (slots s0 .. s0+nslots of src, d0 .. of dst):
+//   dst[d0+slot][p] (+)= scale * sum_i MAT[j][i] * (sum_{k<NSUM} src[s0 + k*sum_slots + slot][p_i])
 // src == dst (in place) is allowed: a thread owns whole pencils.
-template <int SEL, int M, int NPTS, int STRIDE, int C, int NT, int NSUM, bool ADD, bool SCALE>
-__device__ __forceinline__ void sweep(const double *src, int sum_stride, double *dst, int nslots, double scale,
-                                      int tid) {
+template <int SEL, int M, int NPTS, int STRIDE, int C, int NT, int NSUM, bool ADD, bool SCALE, class L>
+__device__ __forceinline__ void sweep(const double *src, int s0, int sum_slots, double *dst, int d0, int nslots,
+                                      double scale, int tid) {
     constexpr int NPEN = NPTS / M;
     const int total = nslots * NPEN * C;
     for (int it = tid; it < total; it += NT) {
@@ -96,13 +121,15 @@ __device__ __forceinline__ void sweep(const double *src, int sum_stride, double 
         const int r = it / C;
         const int pen = r % NPEN;
         const int slot = r / NPEN;
-        const int off = (slot * NPTS + pencil_base<M, STRIDE>(pen)) * C + cell;
+        const int pb = pencil_base<M, STRIDE>(pen);
+        const int so = (s0 + slot) * NPTS + pb;
+        const int dofs = (d0 + slot) * NPTS + pb;
         double in[M];
 #pragma unroll
         for (int i = 0; i < M; ++i) {
-            in[i] = src[off + i * STRIDE * C];
+            in[i] = src[L::at(so + i * STRIDE) * C + cell];
 #pragma unroll
-            for (int k = 1; k < NSUM; ++k) in[i] += src[k * sum_stride + off + i * STRIDE * C];
+            for (int k = 1; k < NSUM; ++k) in[i] += src[L::at(so + k * sum_slots * NPTS + i * STRIDE) * C + cell];
         }
 #pragma unroll
         for (int j = 0; j < M; ++j) {
@@ -110,12 +137,64 @@ __device__ __forceinline__ void sweep(const double *src, int sum_stride, double 
 #pragma unroll
             for (int i = 1; i < M; ++i) acc = fma(mat<SEL>(j * 8 + i), in[i], acc);
             if (SCALE) acc *= scale;
+            double *d = dst + L::at(dofs + j * STRIDE) * C + cell;
             if (ADD)
-                dst[off + j * STRIDE * C] += acc;
+                *d += acc;
             else
-                dst[off + j * STRIDE * C] = acc;
+                *d = acc;
         }
     }
+}
+
+// ---- m x m register tiles: t[y*M + x] ----
+template <int SEL, int M>
+__device__ __forceinline__ void tile_x(double *t) {
+#pragma unroll
+    for (int y = 0; y < M; ++y) {
+        double in[M];
+#pragma unroll
+        for (int i = 0; i < M; ++i) in[i] = t[y * M + i];
+#pragma unroll
+        for (int j = 0; j < M; ++j) {
+            double acc = mat<SEL>(j * 8) * in[0];
+#pragma unroll
+            for (int i = 1; i < M; ++i) acc = fma(mat<SEL>(j * 8 + i), in[i], acc);
+            t[y * M + j] = acc;
+        }
+    }
+}
+template <int SEL, int M>
+__device__ __forceinline__ void tile_y(double *t) {
+#pragma unroll
+    for (int x = 0; x < M; ++x) {
+        double in[M];
+#pragma unroll
+        for (int i = 0; i < M; ++i) in[i] = t[i * M + x];
+#pragma unroll
+        for (int j = 0; j < M; ++j) {
+            double acc = mat<SEL>(j * 8) * in[0];
+#pragma unroll
+            for (int i = 1; i < M; ++i) acc = fma(mat<SEL>(j * 8 + i), in[i], acc);
+            t[j * M + x] = acc;
+        }
+    }
+}
+// tile g (global plane index: P = g*M*M + q) of an array <-> registers; L::PL must be M*M
+template <int M, int C, class L>
+__device__ __forceinline__ void tile_load(const double *a, int g, int cell, double *t) {
+    const int b = L::tile_par(g) * C;
+    const double *pe = a + g * (M * M) * C + cell + b;   // even rows: q ^ 1 = q + 1
+    const double *po = a + g * (M * M) * C + cell - b;   // odd rows:  q ^ 1 = q - 1
+#pragma unroll
+    for (int q = 0; q < M * M; ++q) t[q] = ((q & 1) ? po : pe)[q * C];
+}
+template <int M, int C, class L>
+__device__ __forceinline__ void tile_store(double *a, int g, int cell, const double *t) {
+    const int b = L::tile_par(g) * C;
+    double *pe = a + g * (M * M) * C + cell + b;
+    double *po = a + g * (M * M) * C + cell - b;
+#pragma unroll
+    for (int q = 0; q < M * M; ++q) ((q & 1) ? po : pe)[q * C] = t[q];
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -247,21 +326,35 @@ __device__ __forceinline__ void block_max2(double a, double b, double *red, unsi
 }
 
 // expand slots [0, nslots) of `buf` modal -> nodal in place (Eq. 21), all D axes; ends with a barrier
-template <int D, int M, int C, int NT>
+template <int D, int M, int C, int NT, bool BLK, class L>
 __device__ __forceinline__ void expand_volume(double *buf, int nslots, int tid) {
     constexpr int Np = ipow(M, D);
-    sweep<DG_SEL_V, M, Np, 1, C, NT, 1, false, false>(buf, 0, buf, nslots, 1.0, tid);
-    __syncthreads();
-    sweep<DG_SEL_V, M, Np, M, C, NT, 1, false, false>(buf, 0, buf, nslots, 1.0, tid);
-    __syncthreads();
+    if (BLK) {
+        // x and y in registers, one m x m tile per item
+        const int ntile = nslots * (Np / (M * M));
+        for (int it = tid; it < ntile * C; it += NT) {
+            const int cell = it % C, g = it / C;
+            double t[M * M];
+            tile_load<M, C, L>(buf, g, cell, t);
+            tile_x<DG_SEL_V, M>(t);
+            tile_y<DG_SEL_V, M>(t);
+            tile_store<M, C, L>(buf, g, cell, t);
+        }
+        __syncthreads();
+    } else {
+        sweep<DG_SEL_V, M, Np, 1, C, NT, 1, false, false, L>(buf, 0, 0, buf, 0, nslots, 1.0, tid);
+        __syncthreads();
+        sweep<DG_SEL_V, M, Np, M, C, NT, 1, false, false, L>(buf, 0, 0, buf, 0, nslots, 1.0, tid);
+        __syncthreads();
+    }
     if (D == 3) {
-        sweep<DG_SEL_V, M, Np, M * M, C, NT, 1, false, false>(buf, 0, buf, nslots, 1.0, tid);
+        sweep<DG_SEL_V, M, Np, M * M, C, NT, 1, false, false, L>(buf, 0, 0, buf, 0, nslots, 1.0, tid);
         __syncthreads();
     }
 }
 
 // max c_s and max |v| over the nodal values in RA (Eq. 23 inputs, reading A18)
-template <int D, int M, int C, int NT>
+template <int D, int M, int C, int NT, class L>
 __device__ __forceinline__ void wavespeed_points(const double *RA, double gamma, int *flag, double *red,
                                                  unsigned long long *maxbits, int tid) {
     constexpr int Np = ipow(M, D);
@@ -273,7 +366,7 @@ __device__ __forceinline__ void wavespeed_points(const double *RA, double gamma,
         const int j = it / C;
         double u[Vc];
 #pragma unroll
-        for (int v = 0; v < Vc; ++v) u[v] = RA[(v * Np + j) * C + cell];
+        for (int v = 0; v < Vc; ++v) u[v] = RA[L::at(v * Np + j) * C + cell];
         const Prim<D> q = primitives<D>(u, gamma);
         bad |= !(q.rho > 0.0) || !(q.p > 0.0);
         double v2 = 0.0;
@@ -290,7 +383,7 @@ __device__ __forceinline__ void wavespeed_points(const double *RA, double gamma,
 
 // Own modes of the block's cells, global [r = mode*V + v][cell] -> shared [v][mode][cell].  Thread `tid` keeps
 // cell tid % C; its loads are issued in batches of up to 12 before the first store (one DRAM round trip per batch).
-template <int V, int Np, int C, int NT>
+template <int V, int Np, int C, int NT, class L>
 __device__ __forceinline__ void load_own_modes(const double *__restrict__ w, int ncells, int cg, double *RA, int tid) {
     constexpr int NR = (V * Np * C + NT - 1) / NT;
     constexpr int RB = NR < 12 ? NR : 12;
@@ -306,7 +399,7 @@ __device__ __forceinline__ void load_own_modes(const double *__restrict__ w, int
 #pragma unroll
         for (int j = 0; j < RB; ++j) {
             const int r = tid / C + (k0 + j) * (NT / C);
-            if (k0 + j < NR && r < V * Np) RA[((r % V) * Np + r / V) * C + cl] = t[j];
+            if (k0 + j < NR && r < V * Np) RA[L::at((r % V) * Np + r / V) * C + cl] = t[j];
         }
     }
 }
@@ -331,6 +424,9 @@ struct FaceCfg {
     static constexpr int C = pick_c();
     static constexpr int kSmemBytes = C * FP * 8 + D * C * 4;
     static_assert(kSmemBytes <= kSmemMax, "face kernel: per-cell footprint exceeds shared memory");
+    static constexpr bool SWZ = use_swizzle(M, C);
+    using LV = Lay<M * M, K::Np, SWZ>;          // own modes (volume array)
+    using LF = Lay<K::Nf, K::Nf, SWZ>;          // face arrays: one tile (3D) / one pencil (2D) per slot
 };
 
 template <int D, int M, bool VISC, bool AV, int A>
@@ -338,8 +434,11 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA
                                           int cell0, int tid) {
     using K = Cfg<D, M, VISC, AV>;
     using FK = FaceCfg<D, M, VISC, AV>;
+    using LV = typename FK::LV;
+    using LF = typename FK::LF;
     constexpr int C = FK::C, NT = FK::NT, V = K::V, Vc = K::Vc, Np = K::Np, Nf = K::Nf;
     constexpr bool GRAD = K::GRAD;
+    constexpr bool TILE = K::BLK && (D == 3);    // face arrays are m x m tiles
     constexpr int SA = ipow(M, A);               // stride of axis A inside the cell
     constexpr int oUL = 0, oUR = Vc, oUT = 2 * Vc, oGN = 2 * Vc + V, oGT = 3 * Vc + V;
     const double ih = 1.0 / p.h;
@@ -372,8 +471,7 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA
                 const int base = pencil_base<M, SA>(lt);
                 double own[M];
 #pragma unroll
-                for (int l = 0; l < M; ++l) own[l] = RA[(v * Np + base + l * SA) * C + cell];
-                double *F = RX + lt * C + cell;
+                for (int l = 0; l < M; ++l) own[l] = RA[LV::at(v * Np + base + l * SA) * C + cell];
                 double uL = 0.0, uR = 0.0, ut = 0.0, gn = 0.0;
 #pragma unroll
                 for (int l = 0; l < M; ++l) {
@@ -387,33 +485,56 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA
                     }
                 }
                 if (v < Vc) {
-                    F[(oUL + v) * Nf * C] = uL;
-                    F[(oUR + v) * Nf * C] = uR;
-                    if (GRAD) F[(oGN + v) * Nf * C] = gn * ih;
+                    RX[LF::at((oUL + v) * Nf + lt) * C + cell] = uL;
+                    RX[LF::at((oUR + v) * Nf + lt) * C + cell] = uR;
+                    if (GRAD) RX[LF::at((oGN + v) * Nf + lt) * C + cell] = gn * ih;
                 }
-                if (GRAD) F[(oUT + v) * Nf * C] = ut;
+                if (GRAD) RX[LF::at((oUT + v) * Nf + lt) * C + cell] = ut;
             }
         }
     }
     __syncthreads();
 
-    // F2: transverse modal -> nodal on the face (cell basis kept transversally)
-    if (M > 1) {
-        sweep<DG_SEL_V, M, Nf, 1, C, NT, 1, false, false>(RX, 0, RX, K::NQE, 1.0, tid);
+    // F2: transverse modal -> nodal on the face (cell basis kept transversally), and the
+    // transverse derivatives of the recovered face polynomial
+    if (TILE) {
+        for (int it = tid; it < K::NQE * C; it += NT) {
+            const int cell = it % C, g = it / C;
+            double t[M * M];
+            tile_load<M, C, LF>(RX, g, cell, t);
+            tile_x<DG_SEL_V, M>(t);
+            tile_y<DG_SEL_V, M>(t);
+            tile_store<M, C, LF>(RX, g, cell, t);
+            if (GRAD && g >= oUT && g < oUT + Vc) {
+                double a[M * M];
+#pragma unroll
+                for (int q = 0; q < M * M; ++q) a[q] = t[q];
+                tile_x<DG_SEL_DHAT, M>(a);
+#pragma unroll
+                for (int q = 0; q < M * M; ++q) a[q] *= 2.0 * ih;
+                tile_store<M, C, LF>(RX, oGT + (g - oUT), cell, a);
+                tile_y<DG_SEL_DHAT, M>(t);
+#pragma unroll
+                for (int q = 0; q < M * M; ++q) t[q] *= 2.0 * ih;
+                tile_store<M, C, LF>(RX, oGT + Vc + (g - oUT), cell, t);
+            }
+        }
         __syncthreads();
-        if (D == 3) {
-            sweep<DG_SEL_V, M, Nf, M, C, NT, 1, false, false>(RX, 0, RX, K::NQE, 1.0, tid);
+    } else {
+        if (M > 1) {
+            sweep<DG_SEL_V, M, Nf, 1, C, NT, 1, false, false, LF>(RX, 0, 0, RX, 0, K::NQE, 1.0, tid);
+            __syncthreads();
+            if (D == 3) {
+                sweep<DG_SEL_V, M, Nf, M, C, NT, 1, false, false, LF>(RX, 0, 0, RX, 0, K::NQE, 1.0, tid);
+                __syncthreads();
+            }
+        }
+        if (GRAD) {
+            sweep<DG_SEL_DHAT, M, Nf, 1, C, NT, 1, false, true, LF>(RX, oUT, 0, RX, oGT, Vc, 2.0 * ih, tid);
+            if (D == 3)
+                sweep<DG_SEL_DHAT, M, Nf, M, C, NT, 1, false, true, LF>(RX, oUT, 0, RX, oGT + Vc, Vc, 2.0 * ih, tid);
             __syncthreads();
         }
-    }
-    if (GRAD) {
-        // transverse derivatives of the recovered face polynomial
-        sweep<DG_SEL_DHAT, M, Nf, 1, C, NT, 1, false, true>(RX + oUT * Nf * C, 0, RX + oGT * Nf * C, Vc, 2.0 * ih,
-                                                           tid);
-        if (D == 3)
-            sweep<DG_SEL_DHAT, M, Nf, M, C, NT, 1, false, true>(RX + oUT * Nf * C, 0, RX + (oGT + Vc) * Nf * C, Vc,
-                                                               2.0 * ih, tid);
-        __syncthreads();
     }
 
     // F3: numerical flux at every face point; result overwrites the uL slots
@@ -422,12 +543,11 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA
         for (int it = tid; it < Nf * C; it += NT) {
             const int cell = it % C;
             const int k = it / C;
-            double *F = RX + k * C + cell;
             double uL[Vc], uR[Vc], Fh[Vc];
 #pragma unroll
             for (int v = 0; v < Vc; ++v) {
-                uL[v] = F[(oUL + v) * Nf * C];
-                uR[v] = F[(oUR + v) * Nf * C];
+                uL[v] = RX[LF::at((oUL + v) * Nf + k) * C + cell];
+                uR[v] = RX[LF::at((oUR + v) * Nf + k) * C + cell];
             }
             const Prim<D> qL = primitives<D>(uL, p.gamma);
             const Prim<D> qR = primitives<D>(uR, p.gamma);
@@ -437,11 +557,11 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA
                 double ut[Vc], g[D][D + 2];
 #pragma unroll
                 for (int v = 0; v < Vc; ++v) {
-                    ut[v] = F[(oUT + v) * Nf * C];
+                    ut[v] = RX[LF::at((oUT + v) * Nf + k) * C + cell];
 #pragma unroll
                     for (int b = 0; b < D; ++b) {
                         const int slot = (b == A) ? (oGN + v) : (oGT + (b < A ? b : b - 1) * Vc + v);
-                        g[b][v] = F[slot * Nf * C];
+                        g[b][v] = RX[LF::at(slot * Nf + k) * C + cell];
                     }
                 }
                 const Prim<D> qt = primitives<D>(ut, p.gamma);
@@ -455,7 +575,7 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA
                     ns_flux_sub<D>(qt, g, dv, divv, A, p.gamma, p.nu, p.chi, Fh);
                 }
                 if (AV) {
-                    const double al = F[(oUT + Vc) * Nf * C];
+                    const double al = RX[LF::at((oUT + Vc) * Nf + k) * C + cell];
                     const double cst = sqrt(p.gamma * qt.p * qt.ir);
                     const double eps = fmin(fmax(al, 0.0), p.alpha_max) * cst * p.h / (double)M;   // Eq. 46, A12
 #pragma unroll
@@ -463,22 +583,34 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA
                 }
             }
 #pragma unroll
-            for (int v = 0; v < Vc; ++v) F[(oUL + v) * Nf * C] = Fh[v];
+            for (int v = 0; v < Vc; ++v) RX[LF::at((oUL + v) * Nf + k) * C + cell] = Fh[v];
         }
         if (bad) atomicOr(p.flag, 1);
     }
     __syncthreads();
 
-    // F4: project the face flux on the transverse modes (g_k phi_l(xi_k) of Eq. 20's surface lines)
-    if (M > 1 && D == 3) {
-        sweep<DG_SEL_VTG, M, Nf, 1, C, NT, 1, false, false>(RX, 0, RX, Vc, 1.0, tid);
-        __syncthreads();
-    }
-    // last projection sweep (or the single-point weight g_0^(D-1) = 2^(D-1)) straight to global memory
-    {
+    // F4: project the face flux on the transverse modes (g_k phi_l(xi_k) of Eq. 20's surface lines) -> global
+    double *out = p.flux + (size_t)A * Vc * Nf * p.ncells;
+    if (TILE) {
+        for (int it = tid; it < Vc * C; it += NT) {
+            const int cell = it % C, g = it / C;
+            double t[M * M];
+            tile_load<M, C, LF>(RX, oUL + g, cell, t);
+            tile_x<DG_SEL_VTG, M>(t);
+            tile_y<DG_SEL_VTG, M>(t);
+            if (cell0 + cell < p.ncells) {
+#pragma unroll
+                for (int q = 0; q < M * M; ++q) out[(size_t)(g * Nf + q) * p.ncells + cell0 + cell] = t[q];
+            }
+        }
+    } else {
+        if (M > 1 && D == 3) {
+            sweep<DG_SEL_VTG, M, Nf, 1, C, NT, 1, false, false, LF>(RX, 0, 0, RX, 0, Vc, 1.0, tid);
+            __syncthreads();
+        }
+        // last projection sweep (or the single-point weight g_0^(D-1) = 2^(D-1)) straight to global memory
         constexpr int STR = (D == 3) ? M : 1;
         constexpr int NPEN = Nf / M;
-        double *out = p.flux + (size_t)A * Vc * Nf * p.ncells;
         for (int it = tid; it < Vc * NPEN * C; it += NT) {
             const int cell = it % C;
             const int r = it / C;
@@ -488,7 +620,7 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA
             const int off = v * Nf + pencil_base<M, STR>(pen);
             double in[M];
 #pragma unroll
-            for (int i = 0; i < M; ++i) in[i] = RX[(off + i * STR) * C + cell];
+            for (int i = 0; i < M; ++i) in[i] = RX[LF::at(off + i * STR) * C + cell];
 #pragma unroll
             for (int j = 0; j < M; ++j) {
                 double acc;
@@ -529,7 +661,7 @@ __global__ void __launch_bounds__(256, 3) dg_face_kernel(const DgStageArgs p) {
             nbr[(D - 1) * C + tid] = c + ((iz == p.nz - 1) ? -(p.nz - 1) * pl : pl);
         }
     }
-    load_own_modes<V, Np, C, NT>(p.w_prev, p.ncells, min(cell0 + tid % C, p.ncells - 1), RA, tid);
+    load_own_modes<V, Np, C, NT, typename FK::LV>(p.w_prev, p.ncells, min(cell0 + tid % C, p.ncells - 1), RA, tid);
     __syncthreads();
     face_axis<D, M, VISC, AV, 0>(p, RA, RX, nbr, cell0, tid);
     face_axis<D, M, VISC, AV, 1>(p, RA, RX, nbr, cell0, tid);
@@ -543,13 +675,16 @@ template <int D, int M, bool VISC, bool AV>
 __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(const DgStageArgs p) {
     using K = Cfg<D, M, VISC, AV>;
     constexpr int C = K::C, NT = K::NT, V = K::V, Vc = K::Vc, Np = K::Np;
-    constexpr bool GRAD = K::GRAD;
+    constexpr bool GRAD = K::GRAD, BLK = K::BLK;
+    using L = Lay<M * M, Np, use_swizzle(M, C)>;
+    constexpr int NTILE = Np / (M * M);          // m x m tiles per slot (m in 3D, 1 in 2D)
     extern __shared__ double smem[];
     double *RA = smem;
     double *RX = RA + V * Np * C;
     double *ACC = RX + K::RX * C;
     double *Wk = ACC + V * Np * C;
     double *red = Wk + C;
+    double *sens = red + 2 * (NT / 32);           // [4][NT/32][C] partial sensor sums (AV only)
     const int tid = threadIdx.x;
     const int cell0 = blockIdx.x * C;
 
@@ -594,7 +729,7 @@ __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(co
         Wk[tid] = (S > p.s_onset) ? p.f_w * fmax(0.0, G) : 0.0;
     }
     // own modes -> RA, zero ACC
-    load_own_modes<V, Np, C, NT>(p.w_prev, p.ncells, cg, RA, tid);   // global slot order: r = mode*V + v
+    load_own_modes<V, Np, C, NT, L>(p.w_prev, p.ncells, cg, RA, tid);   // global slot order: r = mode*V + v
     for (int r = tid / C; r < V * Np; r += NT / C) ACC[r * C + cl] = 0.0;
     __syncthreads();
 
@@ -615,7 +750,7 @@ __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(co
                     const int base = (lt / SA) * (SA * M) + (lt % SA);
 #pragma unroll
                     for (int l = 0; l < M; ++l)
-                        ACC[(v * Np + base + l * SA) * C + cl] +=
+                        ACC[L::at(v * Np + base + l * SA) * C + cl] +=
                             pref * (c_tab.Pend[0][l] * Fm[a][k] - c_tab.Pend[1][l] * Fp[a][k]);
                 }
             }
@@ -624,14 +759,31 @@ __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(co
     }
 
     // ---- volume term ----
-    expand_volume<D, M, C, NT>(RA, V, tid);                       // V1: Eq. 21
+    expand_volume<D, M, C, NT, BLK, L>(RA, V, tid);               // V1: Eq. 21
     const double ih = 1.0 / p.h;
     if (GRAD) {
         // V2: gradients at the Gauss points by analytic differentiation of the basis
-        sweep<DG_SEL_DHAT, M, Np, 1, C, NT, 1, false, true>(RA, 0, RX, Vc, 2.0 * ih, tid);
-        sweep<DG_SEL_DHAT, M, Np, M, C, NT, 1, false, true>(RA, 0, RX + Vc * Np * C, Vc, 2.0 * ih, tid);
-        if (D == 3)
-            sweep<DG_SEL_DHAT, M, Np, M * M, C, NT, 1, false, true>(RA, 0, RX + 2 * Vc * Np * C, Vc, 2.0 * ih, tid);
+        if (BLK) {
+            for (int it = tid; it < Vc * NTILE * C; it += NT) {
+                const int cell = it % C, g = it / C;
+                double t[M * M], a[M * M];
+                tile_load<M, C, L>(RA, g, cell, t);
+#pragma unroll
+                for (int q = 0; q < M * M; ++q) a[q] = t[q];
+                tile_x<DG_SEL_DHAT, M>(a);
+#pragma unroll
+                for (int q = 0; q < M * M; ++q) a[q] *= 2.0 * ih;
+                tile_store<M, C, L>(RX, g, cell, a);
+                tile_y<DG_SEL_DHAT, M>(t);
+#pragma unroll
+                for (int q = 0; q < M * M; ++q) t[q] *= 2.0 * ih;
+                tile_store<M, C, L>(RX, Vc * NTILE + g, cell, t);
+            }
+        } else {
+            sweep<DG_SEL_DHAT, M, Np, 1, C, NT, 1, false, true, L>(RA, 0, 0, RX, 0, Vc, 2.0 * ih, tid);
+            sweep<DG_SEL_DHAT, M, Np, M, C, NT, 1, false, true, L>(RA, 0, 0, RX, Vc, Vc, 2.0 * ih, tid);
+        }
+        if (D == 3) sweep<DG_SEL_DHAT, M, Np, M * M, C, NT, 1, false, true, L>(RA, 0, 0, RX, 2 * Vc, Vc, 2.0 * ih, tid);
         __syncthreads();
     }
     {
@@ -642,7 +794,7 @@ __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(co
             const int j = it / C;
             double u[Vc];
 #pragma unroll
-            for (int v = 0; v < Vc; ++v) u[v] = RA[(v * Np + j) * C + cell];
+            for (int v = 0; v < Vc; ++v) u[v] = RA[L::at(v * Np + j) * C + cell];
             const Prim<D> q = primitives<D>(u, p.gamma);
             bad |= !(q.rho > 0.0) || !(q.p > 0.0);
             double g[D][D + 2], dv[D][D];
@@ -651,18 +803,18 @@ __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(co
 #pragma unroll
                 for (int b = 0; b < D; ++b)
 #pragma unroll
-                    for (int v = 0; v < Vc; ++v) g[b][v] = RX[((b * Vc + v) * Np + j) * C + cell];
+                    for (int v = 0; v < Vc; ++v) g[b][v] = RX[L::at((b * Vc + v) * Np + j) * C + cell];
                 velocity_gradient<D>(q, g, dv);
 #pragma unroll
                 for (int b = 0; b < D; ++b) divv += dv[b][b];
             }
             if (AV) {
-                const double al = RA[(Vc * Np + j) * C + cell];
+                const double al = RA[L::at(Vc * Np + j) * C + cell];
                 const double cs = sqrt(p.gamma * q.p * q.ir);
                 eps = fmin(fmax(al, 0.0), p.alpha_max) * cs * p.h / (double)M;        // Eq. 46, A17
                 // Eq. 43-45: shock source + wiggle source - decay; stored pre-scaled by h/2 for the projection
                 const double src = p.f_v * fmax(0.0, -divv) + Wk[cell] - al * ((double)M * cs / (p.f_tau * p.h));
-                RA[(Vc * Np + j) * C + cell] = 0.5 * p.h * src;
+                RA[L::at(Vc * Np + j) * C + cell] = 0.5 * p.h * src;
             }
 #pragma unroll
             for (int a = 0; a < D; ++a) {
@@ -674,68 +826,87 @@ __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(co
                     for (int v = 0; v < Vc; ++v) F[v] -= eps * g[a][v];
                 }
 #pragma unroll
-                for (int v = 0; v < Vc; ++v) RX[((a * Vc + v) * Np + j) * C + cell] = F[v];
+                for (int v = 0; v < Vc; ++v) RX[L::at((a * Vc + v) * Np + j) * C + cell] = F[v];
             }
         }
         if (bad) atomicOr(p.flag, 1);
     }
     __syncthreads();
-    // V4: weak-form derivative in nodal space, N = sum_a S_a G_a
-    sweep<DG_SEL_S, M, Np, 1, C, NT, 1, false, false>(RX, 0, RX, Vc, 1.0, tid);
-    sweep<DG_SEL_S, M, Np, M, C, NT, 1, false, false>(RX + Vc * Np * C, 0, RX + Vc * Np * C, Vc, 1.0, tid);
-    if (D == 3)
-        sweep<DG_SEL_S, M, Np, M * M, C, NT, 1, false, false>(RX + 2 * Vc * Np * C, 0, RX + 2 * Vc * Np * C, Vc, 1.0,
-                                                            tid);
-    __syncthreads();
-    // V5: projection on the modes, dw += pref * (x) VtG N
+    // V4 + V5: weak-form derivative in nodal space, N = sum_a S_a G_a, then projection on the modes,
+    //          dw += pref * (x)_a VtG N; alpha row: projection of the source only
     {
         const double pref = (D == 3 ? 0.25 : 0.5) * ih;
-        sweep<DG_SEL_VTG, M, Np, 1, C, NT, D, false, false>(RX, Vc * Np * C, RX, Vc, 1.0, tid);
-        if (AV) sweep<DG_SEL_VTG, M, Np, 1, C, NT, 1, false, false>(RA + Vc * Np * C, 0, RA + Vc * Np * C, 1, 1.0, tid);
-        __syncthreads();
-        if (D == 3) {
-            sweep<DG_SEL_VTG, M, Np, M, C, NT, 1, false, false>(RX, 0, RX, Vc, 1.0, tid);
-            if (AV)
-                sweep<DG_SEL_VTG, M, Np, M, C, NT, 1, false, false>(RA + Vc * Np * C, 0, RA + Vc * Np * C, 1, 1.0, tid);
+        if (BLK) {
+            if (D == 3) {
+                sweep<DG_SEL_S, M, Np, M * M, C, NT, 1, false, false, L>(RX, 2 * Vc, 0, RX, 2 * Vc, Vc, 1.0, tid);
+                __syncthreads();
+            }
+            // per m x m tile: S_x G_x + S_y G_y (+ S_z G_z), projected along x and y in registers
+            for (int it = tid; it < V * NTILE * C; it += NT) {
+                const int cell = it % C, g = it / C;
+                double n[M * M];
+                if (g < Vc * NTILE) {
+                    double b[M * M];
+                    tile_load<M, C, L>(RX, g, cell, n);
+                    tile_x<DG_SEL_S, M>(n);
+                    tile_load<M, C, L>(RX, Vc * NTILE + g, cell, b);
+                    tile_y<DG_SEL_S, M>(b);
+#pragma unroll
+                    for (int q = 0; q < M * M; ++q) n[q] += b[q];
+                    if (D == 3) {
+                        tile_load<M, C, L>(RX, 2 * Vc * NTILE + g, cell, b);
+#pragma unroll
+                        for (int q = 0; q < M * M; ++q) n[q] += b[q];
+                    }
+                } else {
+                    tile_load<M, C, L>(RA, g, cell, n);      // alpha source (slot Vc of RA)
+                }
+                tile_x<DG_SEL_VTG, M>(n);
+                tile_y<DG_SEL_VTG, M>(n);
+                if (D == 3) {
+                    if (g < Vc * NTILE)
+                        tile_store<M, C, L>(RX, g, cell, n);
+                    else
+                        tile_store<M, C, L>(RA, g, cell, n);
+                } else {
+                    double acc[M * M];
+                    tile_load<M, C, L>(ACC, g, cell, acc);
+#pragma unroll
+                    for (int q = 0; q < M * M; ++q) acc[q] = fma(pref, n[q], acc[q]);
+                    tile_store<M, C, L>(ACC, g, cell, acc);
+                }
+            }
+            __syncthreads();
+            if (D == 3) {
+                sweep<DG_SEL_VTG, M, Np, M * M, C, NT, 1, true, true, L>(RX, 0, 0, ACC, 0, Vc, pref, tid);
+                if (AV) sweep<DG_SEL_VTG, M, Np, M * M, C, NT, 1, true, true, L>(RA, Vc, 0, ACC, Vc, 1, pref, tid);
+                __syncthreads();
+            }
+        } else {
+            sweep<DG_SEL_S, M, Np, 1, C, NT, 1, false, false, L>(RX, 0, 0, RX, 0, Vc, 1.0, tid);
+            sweep<DG_SEL_S, M, Np, M, C, NT, 1, false, false, L>(RX, Vc, 0, RX, Vc, Vc, 1.0, tid);
+            if (D == 3) sweep<DG_SEL_S, M, Np, M * M, C, NT, 1, false, false, L>(RX, 2 * Vc, 0, RX, 2 * Vc, Vc, 1.0, tid);
+            __syncthreads();
+            sweep<DG_SEL_VTG, M, Np, 1, C, NT, D, false, false, L>(RX, 0, Vc, RX, 0, Vc, 1.0, tid);
+            if (AV) sweep<DG_SEL_VTG, M, Np, 1, C, NT, 1, false, false, L>(RA, Vc, 0, RA, Vc, 1, 1.0, tid);
+            __syncthreads();
+            if (D == 3) {
+                sweep<DG_SEL_VTG, M, Np, M, C, NT, 1, false, false, L>(RX, 0, 0, RX, 0, Vc, 1.0, tid);
+                if (AV) sweep<DG_SEL_VTG, M, Np, M, C, NT, 1, false, false, L>(RA, Vc, 0, RA, Vc, 1, 1.0, tid);
+                __syncthreads();
+            }
+            constexpr int SL = (D == 3) ? M * M : M;
+            sweep<DG_SEL_VTG, M, Np, SL, C, NT, 1, true, true, L>(RX, 0, 0, ACC, 0, Vc, pref, tid);
+            if (AV) sweep<DG_SEL_VTG, M, Np, SL, C, NT, 1, true, true, L>(RA, Vc, 0, ACC, Vc, 1, pref, tid);
             __syncthreads();
         }
-        constexpr int SL = (D == 3) ? M * M : M;
-        sweep<DG_SEL_VTG, M, Np, SL, C, NT, 1, true, true>(RX, 0, ACC, Vc, pref, tid);
-        if (AV) sweep<DG_SEL_VTG, M, Np, SL, C, NT, 1, true, true>(RA + Vc * Np * C, 0, ACC + Vc * Np * C, 1, pref, tid);
-        __syncthreads();
     }
 
-    // ---- sensor bookkeeping (Eq. 42, 45; reading A13/A15): density row of w and dw/dt ----
-    if (AV && p.do_sensor && tid < C && cell0 + tid < p.ncells) {
-        const int c = cell0 + tid;
-        double sA = 0.0, sB = 0.0, dA = 0.0, dB = 0.0;
-        for (int mode = 0; mode < Np; ++mode) {
-            int rem = mode, top = 0;
-#pragma unroll
-            for (int a = 0; a < D; ++a) {
-                top |= (rem % M == M - 1);
-                rem /= M;
-            }
-            const double w = p.w_prev[(size_t)(mode * V) * p.ncells + c];
-            const double wd = ACC[mode * C + tid];
-            sB = fma(w, w, sB);
-            dB = fma(w, wd, dB);
-            if (top && M > 1) {
-                sA = fma(w, w, sA);
-                dA = fma(w, wd, dA);
-            }
-        }
-        p.sens_new[c] = sA / sB;
-        p.sens_new[p.ncells + c] = (sA > 0.0) ? (2.0 * dA / sA - 2.0 * dB / sB) : 0.0;
-    }
-    if (AV && p.commit_sensor && tid < C && cell0 + tid < p.ncells) {
-        const int c = cell0 + tid;
-        p.sens_prev[c] = p.sens_new[c];
-        p.sens_prev[p.ncells + c] = p.sens_new[p.ncells + c];
-    }
-
-    // ---- stage combine ----
+    // ---- stage combine + shock-sensor sums (Eq. 42, 45; readings A13/A15) ----
+    // The sensor is evaluated on stage 1 only, where w_prev == w_n: the density rows of w^n and dw/dt pass through
+    // the combine loop; partial sums per thread are reduced per cell in a fixed order.
     const double cdt = p.rhs_only ? 1.0 : p.rk_c * p.scal[0];
+    double sA = 0.0, sB = 0.0, dA = 0.0, dB = 0.0;
     {
         constexpr int NR = (V * Np * C + NT - 1) / NT;
         constexpr int RB = NR < 6 ? NR : 6;
@@ -758,20 +929,67 @@ __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(co
                 const int r = tid / C + (k0 + j) * (NT / C);
                 if (k0 + j < NR && r < V * Np) {
                     const int mode = r / V, v = r % V;
-                    const double L = ACC[(v * Np + mode) * C + cl];
-                    double wnew = L;
-                    if (!p.rhs_only) wnew = fma(cdt, L, fma(p.rk_b, wp[j], p.rk_a * wn[j]));
+                    const double Ld = ACC[L::at(v * Np + mode) * C + cl];
+                    double wnew = Ld;
+                    if (!p.rhs_only) wnew = fma(cdt, Ld, fma(p.rk_b, wp[j], p.rk_a * wn[j]));
                     if (active) p.w_out[(size_t)r * p.ncells + cg] = wnew;
-                    if (p.do_wavespeed) RA[(v * Np + mode) * C + cl] = wnew;
+                    if (p.do_wavespeed) RA[L::at(v * Np + mode) * C + cl] = wnew;
+                    if (AV && p.do_sensor && v == 0) {
+                        int rem = mode, top = 0;
+#pragma unroll
+                        for (int a = 0; a < D; ++a) {
+                            top |= (rem % M == M - 1);
+                            rem /= M;
+                        }
+                        const double w = wn[j];
+                        sB = fma(w, w, sB);
+                        dB = fma(w, Ld, dB);
+                        if (top && M > 1) {
+                            sA = fma(w, w, sA);
+                            dA = fma(w, Ld, dA);
+                        }
+                    }
                 }
             }
         }
     }
+    if (AV && p.do_sensor) {
+        // lanes of a warp that share a cell (lane = cl + C*j), then one partial per warp and cell in `sens`
+        constexpr int NW = NT / 32;
+#pragma unroll
+        for (int o = C; o < 32; o <<= 1) {
+            sA += __shfl_xor_sync(0xffffffffu, sA, o);
+            sB += __shfl_xor_sync(0xffffffffu, sB, o);
+            dA += __shfl_xor_sync(0xffffffffu, dA, o);
+            dB += __shfl_xor_sync(0xffffffffu, dB, o);
+        }
+        if ((tid & 31) < C) {
+            sens[(0 * NW + tid / 32) * C + cl] = sA;
+            sens[(1 * NW + tid / 32) * C + cl] = sB;
+            sens[(2 * NW + tid / 32) * C + cl] = dA;
+            sens[(3 * NW + tid / 32) * C + cl] = dB;
+        }
+        __syncthreads();
+        if (tid < C && cell0 + tid < p.ncells) {
+            double s[4] = {0.0, 0.0, 0.0, 0.0};
+            for (int k = 0; k < NW; ++k)
+#pragma unroll
+                for (int i = 0; i < 4; ++i) s[i] += sens[(i * NW + k) * C + tid];
+            const int c = cell0 + tid;
+            p.sens_new[c] = s[0] / s[1];
+            p.sens_new[p.ncells + c] = (s[0] > 0.0) ? (2.0 * s[2] / s[0] - 2.0 * s[3] / s[1]) : 0.0;
+        }
+    }
+    if (AV && p.commit_sensor && tid < C && cell0 + tid < p.ncells) {
+        const int c = cell0 + tid;
+        p.sens_prev[c] = p.sens_new[c];
+        p.sens_prev[p.ncells + c] = p.sens_new[p.ncells + c];
+    }
     // ---- wave speeds of the new state for the next step's Eq. 23 ----
     if (p.do_wavespeed) {
         __syncthreads();
-        expand_volume<D, M, C, NT>(RA, Vc, tid);
-        wavespeed_points<D, M, C, NT>(RA, p.gamma, p.flag, red, p.maxbits, tid);
+        expand_volume<D, M, C, NT, BLK, L>(RA, Vc, tid);
+        wavespeed_points<D, M, C, NT, L>(RA, p.gamma, p.flag, red, p.maxbits, tid);
     }
 }
 
@@ -780,21 +998,16 @@ template <int D, int M, bool VISC, bool AV>
 __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_wavespeed_kernel(const DgStageArgs p) {
     using K = Cfg<D, M, VISC, AV>;
     constexpr int C = K::C, NT = K::NT, V = K::V, Vc = K::Vc, Np = K::Np;
+    using L = Lay<M * M, Np, use_swizzle(M, C)>;
     extern __shared__ double smem[];
     double *RA = smem;
     double *red = RA + V * Np * C + K::RX * C + V * Np * C + C;
     const int tid = threadIdx.x;
     const int cell0 = blockIdx.x * C;
-    for (int it = tid; it < Vc * Np * C; it += NT) {
-        const int cell = it % C;
-        const int r = it / C;   // mode*Vc + v
-        const int mode = r / Vc, v = r % Vc;
-        const int cg = min(cell0 + cell, p.ncells - 1);
-        RA[(v * Np + mode) * C + cell] = p.w_prev[(size_t)(mode * V + v) * p.ncells + cg];
-    }
+    load_own_modes<V, Np, C, NT, L>(p.w_prev, p.ncells, min(cell0 + tid % C, p.ncells - 1), RA, tid);
     __syncthreads();
-    expand_volume<D, M, C, NT>(RA, Vc, tid);
-    wavespeed_points<D, M, C, NT>(RA, p.gamma, p.flag, red, p.maxbits, tid);
+    expand_volume<D, M, C, NT, K::BLK, L>(RA, Vc, tid);
+    wavespeed_points<D, M, C, NT, L>(RA, p.gamma, p.flag, red, p.maxbits, tid);
 }
 
 }  // namespace dgk

@@ -30,10 +30,16 @@
 #define DG_SEL_VTG 3
 
 #ifndef DG_STAGE_NT
-#define DG_STAGE_NT 256
+#define DG_STAGE_NT 512
 #endif
 #ifndef DG_STAGE_MINB
-#define DG_STAGE_MINB 2
+#define DG_STAGE_MINB 1
+#endif
+#ifndef DG_FACE_NT
+#define DG_FACE_NT 256
+#endif
+#ifndef DG_FACE_MINB
+#define DG_FACE_MINB 2
 #endif
 
 __constant__ DgTables c_tab;
@@ -59,14 +65,15 @@ struct Cfg {
     static constexpr int RX = D * Vc * Np;                         // gradients -> fluxes (in place)
     static constexpr int FP = 2 * V * Np + RX;                     // doubles per cell
     static constexpr int NT = DG_STAGE_NT;
+    // W^K per cell, wave-speed reduction scratch, partial sensor sums
+    static constexpr int extra_doubles(int c) { return c + 2 * (NT / 32) + (AV ? 4 * (NT / 32) * c : 0); }
     static constexpr int pick_c() {
         int c = 32;
-        while (c > 1 && c * FP * 8 > kSmemBudget) c >>= 1;
+        while (c > 1 && (c * FP + extra_doubles(c)) * 8 > kSmemBudget) c >>= 1;
         return c;
     }
     static constexpr int C = pick_c();
-    // W^K per cell, wave-speed reduction scratch, partial sensor sums
-    static constexpr int kExtraDoubles = C + 2 * (NT / 32) + (AV ? 4 * (NT / 32) * C : 0);
+    static constexpr int kExtraDoubles = extra_doubles(C);
     static constexpr int kSmemBytes = (C * FP + kExtraDoubles) * 8;
     static_assert(kSmemBytes <= kSmemMax, "per-cell footprint exceeds shared memory");
     // A tile of m x m points (the two fastest axes) is swept in registers when it fits (m <= 5).
@@ -86,6 +93,12 @@ struct Lay {
             return P ^ (par & 1);
         }
         return P;
+    }
+    // same as at(slot*NPTS + j); with `slot` a compile-time constant after unrolling this needs one runtime XOR per j
+    // (NPTS / PL is even or 1 whenever SWZ is on)
+    static __device__ __forceinline__ int at2(int slot, int j) {
+        if (SWZ) return slot * NPTS + (j ^ ((j / PL + slot) & 1));
+        return slot * NPTS + j;
     }
     // parity of tile g (PL points per tile): rows q and q^1 of the tile are exchanged when it is 1
     static __device__ __forceinline__ int tile_par(int g) {
@@ -115,21 +128,19 @@ template <int SEL, int M, int NPTS, int STRIDE, int C, int NT, int NSUM, bool AD
 __device__ __forceinline__ void sweep(const double *src, int s0, int sum_slots, double *dst, int d0, int nslots,
                                       double scale, int tid) {
     constexpr int NPEN = NPTS / M;
-    const int total = nslots * NPEN * C;
-    for (int it = tid; it < total; it += NT) {
-        const int cell = it % C;
-        const int r = it / C;
+    static_assert(NT % C == 0, "threads per block must be a multiple of cells per block");
+    const int cell = tid % C;
+    const int total = nslots * NPEN;
+    for (int r = tid / C; r < total; r += NT / C) {
         const int pen = r % NPEN;
         const int slot = r / NPEN;
         const int pb = pencil_base<M, STRIDE>(pen);
-        const int so = (s0 + slot) * NPTS + pb;
-        const int dofs = (d0 + slot) * NPTS + pb;
         double in[M];
 #pragma unroll
         for (int i = 0; i < M; ++i) {
-            in[i] = src[L::at(so + i * STRIDE) * C + cell];
+            in[i] = src[L::at2(s0 + slot, pb + i * STRIDE) * C + cell];
 #pragma unroll
-            for (int k = 1; k < NSUM; ++k) in[i] += src[L::at(so + k * sum_slots * NPTS + i * STRIDE) * C + cell];
+            for (int k = 1; k < NSUM; ++k) in[i] += src[L::at2(s0 + k * sum_slots + slot, pb + i * STRIDE) * C + cell];
         }
 #pragma unroll
         for (int j = 0; j < M; ++j) {
@@ -137,7 +148,7 @@ __device__ __forceinline__ void sweep(const double *src, int s0, int sum_slots, 
 #pragma unroll
             for (int i = 1; i < M; ++i) acc = fma(mat<SEL>(j * 8 + i), in[i], acc);
             if (SCALE) acc *= scale;
-            double *d = dst + L::at(dofs + j * STRIDE) * C + cell;
+            double *d = dst + L::at2(d0 + slot, pb + j * STRIDE) * C + cell;
             if (ADD)
                 *d += acc;
             else
@@ -366,7 +377,7 @@ __device__ __forceinline__ void wavespeed_points(const double *RA, double gamma,
         const int j = it / C;
         double u[Vc];
 #pragma unroll
-        for (int v = 0; v < Vc; ++v) u[v] = RA[L::at(v * Np + j) * C + cell];
+        for (int v = 0; v < Vc; ++v) u[v] = RA[L::at2(v, j) * C + cell];
         const Prim<D> q = primitives<D>(u, gamma);
         bad |= !(q.rho > 0.0) || !(q.p > 0.0);
         double v2 = 0.0;
@@ -399,7 +410,7 @@ __device__ __forceinline__ void load_own_modes(const double *__restrict__ w, int
 #pragma unroll
         for (int j = 0; j < RB; ++j) {
             const int r = tid / C + (k0 + j) * (NT / C);
-            if (k0 + j < NR && r < V * Np) RA[L::at((r % V) * Np + r / V) * C + cl] = t[j];
+            if (k0 + j < NR && r < V * Np) RA[L::at2(r % V, r / V) * C + cl] = t[j];
         }
     }
 }
@@ -414,11 +425,11 @@ __device__ __forceinline__ void load_own_modes(const double *__restrict__ w, int
 template <int D, int M, bool VISC, bool AV>
 struct FaceCfg {
     using K = Cfg<D, M, VISC, AV>;
-    static constexpr int NT = 256;
+    static constexpr int NT = DG_FACE_NT;
     static constexpr int FP = K::V * K::Np + K::NQ * K::Nf;       // doubles per cell: own modes + one face
     static constexpr int pick_c() {
         int c = 32;
-        while (c > 1 && c * FP * 8 > 72 * 1024) c >>= 1;          // three resident blocks per SM
+        while (c > 1 && c * FP * 8 > (227 * 1024) / DG_FACE_MINB - 2048) c >>= 1;   // DG_FACE_MINB resident blocks per SM
         return c;
     }
     static constexpr int C = pick_c();
@@ -436,7 +447,7 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA
     using FK = FaceCfg<D, M, VISC, AV>;
     using LV = typename FK::LV;
     using LF = typename FK::LF;
-    constexpr int C = FK::C, NT = FK::NT, V = K::V, Vc = K::Vc, Np = K::Np, Nf = K::Nf;
+    constexpr int C = FK::C, NT = FK::NT, V = K::V, Vc = K::Vc, Nf = K::Nf;
     constexpr bool GRAD = K::GRAD;
     constexpr bool TILE = K::BLK && (D == 3);    // face arrays are m x m tiles
     constexpr int SA = ipow(M, A);               // stride of axis A inside the cell
@@ -471,7 +482,7 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA
                 const int base = pencil_base<M, SA>(lt);
                 double own[M];
 #pragma unroll
-                for (int l = 0; l < M; ++l) own[l] = RA[LV::at(v * Np + base + l * SA) * C + cell];
+                for (int l = 0; l < M; ++l) own[l] = RA[LV::at2(v, base + l * SA) * C + cell];
                 double uL = 0.0, uR = 0.0, ut = 0.0, gn = 0.0;
 #pragma unroll
                 for (int l = 0; l < M; ++l) {
@@ -485,11 +496,11 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA
                     }
                 }
                 if (v < Vc) {
-                    RX[LF::at((oUL + v) * Nf + lt) * C + cell] = uL;
-                    RX[LF::at((oUR + v) * Nf + lt) * C + cell] = uR;
-                    if (GRAD) RX[LF::at((oGN + v) * Nf + lt) * C + cell] = gn * ih;
+                    RX[LF::at2(oUL + v, lt) * C + cell] = uL;
+                    RX[LF::at2(oUR + v, lt) * C + cell] = uR;
+                    if (GRAD) RX[LF::at2(oGN + v, lt) * C + cell] = gn * ih;
                 }
-                if (GRAD) RX[LF::at((oUT + v) * Nf + lt) * C + cell] = ut;
+                if (GRAD) RX[LF::at2(oUT + v, lt) * C + cell] = ut;
             }
         }
     }
@@ -546,8 +557,8 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA
             double uL[Vc], uR[Vc], Fh[Vc];
 #pragma unroll
             for (int v = 0; v < Vc; ++v) {
-                uL[v] = RX[LF::at((oUL + v) * Nf + k) * C + cell];
-                uR[v] = RX[LF::at((oUR + v) * Nf + k) * C + cell];
+                uL[v] = RX[LF::at2(oUL + v, k) * C + cell];
+                uR[v] = RX[LF::at2(oUR + v, k) * C + cell];
             }
             const Prim<D> qL = primitives<D>(uL, p.gamma);
             const Prim<D> qR = primitives<D>(uR, p.gamma);
@@ -557,11 +568,11 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA
                 double ut[Vc], g[D][D + 2];
 #pragma unroll
                 for (int v = 0; v < Vc; ++v) {
-                    ut[v] = RX[LF::at((oUT + v) * Nf + k) * C + cell];
+                    ut[v] = RX[LF::at2(oUT + v, k) * C + cell];
 #pragma unroll
                     for (int b = 0; b < D; ++b) {
                         const int slot = (b == A) ? (oGN + v) : (oGT + (b < A ? b : b - 1) * Vc + v);
-                        g[b][v] = RX[LF::at(slot * Nf + k) * C + cell];
+                        g[b][v] = RX[LF::at2(slot, k) * C + cell];
                     }
                 }
                 const Prim<D> qt = primitives<D>(ut, p.gamma);
@@ -575,7 +586,7 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA
                     ns_flux_sub<D>(qt, g, dv, divv, A, p.gamma, p.nu, p.chi, Fh);
                 }
                 if (AV) {
-                    const double al = RX[LF::at((oUT + Vc) * Nf + k) * C + cell];
+                    const double al = RX[LF::at2(oUT + Vc, k) * C + cell];
                     const double cst = sqrt(p.gamma * qt.p * qt.ir);
                     const double eps = fmin(fmax(al, 0.0), p.alpha_max) * cst * p.h / (double)M;   // Eq. 46, A12
 #pragma unroll
@@ -583,7 +594,7 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA
                 }
             }
 #pragma unroll
-            for (int v = 0; v < Vc; ++v) RX[LF::at((oUL + v) * Nf + k) * C + cell] = Fh[v];
+            for (int v = 0; v < Vc; ++v) RX[LF::at2(oUL + v, k) * C + cell] = Fh[v];
         }
         if (bad) atomicOr(p.flag, 1);
     }
@@ -620,7 +631,7 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA
             const int off = v * Nf + pencil_base<M, STR>(pen);
             double in[M];
 #pragma unroll
-            for (int i = 0; i < M; ++i) in[i] = RX[LF::at(off + i * STR) * C + cell];
+            for (int i = 0; i < M; ++i) in[i] = RX[LF::at2(v, pencil_base<M, STR>(pen) + i * STR) * C + cell];
 #pragma unroll
             for (int j = 0; j < M; ++j) {
                 double acc;
@@ -639,7 +650,7 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA
 }
 
 template <int D, int M, bool VISC, bool AV>
-__global__ void __launch_bounds__(256, 3) dg_face_kernel(const DgStageArgs p) {
+__global__ void __launch_bounds__(DG_FACE_NT, DG_FACE_MINB) dg_face_kernel(const DgStageArgs p) {
     using K = Cfg<D, M, VISC, AV>;
     using FK = FaceCfg<D, M, VISC, AV>;
     constexpr int C = FK::C, NT = FK::NT, V = K::V, Np = K::Np;
@@ -750,7 +761,7 @@ __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(co
                     const int base = (lt / SA) * (SA * M) + (lt % SA);
 #pragma unroll
                     for (int l = 0; l < M; ++l)
-                        ACC[L::at(v * Np + base + l * SA) * C + cl] +=
+                        ACC[L::at2(v, base + l * SA) * C + cl] +=
                             pref * (c_tab.Pend[0][l] * Fm[a][k] - c_tab.Pend[1][l] * Fp[a][k]);
                 }
             }
@@ -794,7 +805,7 @@ __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(co
             const int j = it / C;
             double u[Vc];
 #pragma unroll
-            for (int v = 0; v < Vc; ++v) u[v] = RA[L::at(v * Np + j) * C + cell];
+            for (int v = 0; v < Vc; ++v) u[v] = RA[L::at2(v, j) * C + cell];
             const Prim<D> q = primitives<D>(u, p.gamma);
             bad |= !(q.rho > 0.0) || !(q.p > 0.0);
             double g[D][D + 2], dv[D][D];
@@ -803,18 +814,18 @@ __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(co
 #pragma unroll
                 for (int b = 0; b < D; ++b)
 #pragma unroll
-                    for (int v = 0; v < Vc; ++v) g[b][v] = RX[L::at((b * Vc + v) * Np + j) * C + cell];
+                    for (int v = 0; v < Vc; ++v) g[b][v] = RX[L::at2(b * Vc + v, j) * C + cell];
                 velocity_gradient<D>(q, g, dv);
 #pragma unroll
                 for (int b = 0; b < D; ++b) divv += dv[b][b];
             }
             if (AV) {
-                const double al = RA[L::at(Vc * Np + j) * C + cell];
+                const double al = RA[L::at2(Vc, j) * C + cell];
                 const double cs = sqrt(p.gamma * q.p * q.ir);
                 eps = fmin(fmax(al, 0.0), p.alpha_max) * cs * p.h / (double)M;        // Eq. 46, A17
                 // Eq. 43-45: shock source + wiggle source - decay; stored pre-scaled by h/2 for the projection
                 const double src = p.f_v * fmax(0.0, -divv) + Wk[cell] - al * ((double)M * cs / (p.f_tau * p.h));
-                RA[L::at(Vc * Np + j) * C + cell] = 0.5 * p.h * src;
+                RA[L::at2(Vc, j) * C + cell] = 0.5 * p.h * src;
             }
 #pragma unroll
             for (int a = 0; a < D; ++a) {
@@ -826,7 +837,7 @@ __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(co
                     for (int v = 0; v < Vc; ++v) F[v] -= eps * g[a][v];
                 }
 #pragma unroll
-                for (int v = 0; v < Vc; ++v) RX[L::at((a * Vc + v) * Np + j) * C + cell] = F[v];
+                for (int v = 0; v < Vc; ++v) RX[L::at2(a * Vc + v, j) * C + cell] = F[v];
             }
         }
         if (bad) atomicOr(p.flag, 1);
@@ -929,11 +940,11 @@ __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(co
                 const int r = tid / C + (k0 + j) * (NT / C);
                 if (k0 + j < NR && r < V * Np) {
                     const int mode = r / V, v = r % V;
-                    const double Ld = ACC[L::at(v * Np + mode) * C + cl];
+                    const double Ld = ACC[L::at2(v, mode) * C + cl];
                     double wnew = Ld;
                     if (!p.rhs_only) wnew = fma(cdt, Ld, fma(p.rk_b, wp[j], p.rk_a * wn[j]));
                     if (active) p.w_out[(size_t)r * p.ncells + cg] = wnew;
-                    if (p.do_wavespeed) RA[L::at(v * Np + mode) * C + cl] = wnew;
+                    if (p.do_wavespeed) RA[L::at2(v, mode) * C + cl] = wnew;
                     if (AV && p.do_sensor && v == 0) {
                         int rem = mode, top = 0;
 #pragma unroll

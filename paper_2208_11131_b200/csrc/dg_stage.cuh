@@ -211,6 +211,27 @@ __device__ __forceinline__ void tile_store(double *a, int g, int cell, const dou
 // ---------------------------------------------------------------------------------------------------
 // point-wise physics (Eq. 1-5; 106; 311-323 Eq. 37-39; 375-407 Eq. 43-46)
 // ---------------------------------------------------------------------------------------------------
+// Reciprocal and square root without the IEEE slow path: hardware seed (>= 20 bits) + Newton steps to ~1 ulp.
+// (fp64 division / sqrt compile to ~20-instruction sequences with a branch; these are 6-9 fused operations.)
+__device__ __forceinline__ double fast_rcp(double x) {
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    r = fma(r, fma(-x, r, 1.0), r);
+    r = fma(r, fma(-x, r, 1.0), r);
+    return r;
+}
+__device__ __forceinline__ double fast_sqrt(double x) {
+    if (!(x > 1e-280) || !(x < 1e280)) return sqrt(x);   // zero, negative, NaN, extreme magnitudes: library path
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double hx = 0.5 * x;
+    y = y * fma(-hx * y, y, 1.5);
+    y = y * fma(-hx * y, y, 1.5);
+    double s = x * y;
+    s = fma(fma(-s, s, x), 0.5 * y, s);
+    return s;
+}
+
 template <int D>
 struct Prim {
     double rho, ir, v[D], p, e;
@@ -220,7 +241,7 @@ template <int D>
 __device__ __forceinline__ Prim<D> primitives(const double *u, double gamma) {
     Prim<D> q;
     q.rho = u[0];
-    q.ir = 1.0 / q.rho;
+    q.ir = fast_rcp(q.rho);
     double v2 = 0.0;
 #pragma unroll
     for (int b = 0; b < D; ++b) {
@@ -246,8 +267,8 @@ __device__ __forceinline__ void euler_flux(const double *u, const Prim<D> &q, in
 template <int D>
 __device__ __forceinline__ void hllc_flux(const double *uL, const double *uR, const Prim<D> &L, const Prim<D> &R,
                                           int a, double gamma, double *F) {
-    const double cL = sqrt(gamma * L.p * L.ir);
-    const double cR = sqrt(gamma * R.p * R.ir);
+    const double cL = fast_sqrt(gamma * L.p * L.ir);
+    const double cR = fast_sqrt(gamma * R.p * R.ir);
     const double vnL = L.v[a], vnR = R.v[a];
     const double SL = fmin(vnL - cL, vnR - cR);
     const double SR = fmax(vnL + cL, vnR + cR);
@@ -261,7 +282,7 @@ __device__ __forceinline__ void hllc_flux(const double *uL, const double *uR, co
     }
     const double mL = L.rho * (SL - vnL);
     const double mR = R.rho * (SR - vnR);
-    const double Sstar = (R.p - L.p + mL * vnL - mR * vnR) / (mL - mR);
+    const double Sstar = (R.p - L.p + mL * vnL - mR * vnR) * fast_rcp(mL - mR);
     // F_K + S_K (U*_K - U_K), K = L if S* >= 0 else R
     const bool left = (Sstar >= 0.0);
     const double *u = left ? uL : uR;
@@ -271,14 +292,14 @@ __device__ __forceinline__ void hllc_flux(const double *uL, const double *uR, co
     const double mK = left ? mL : mR;
     double f[D + 2];
     euler_flux<D>(u, K, a, f);
-    const double fac = mK / (S - Sstar);
+    const double fac = mK * fast_rcp(S - Sstar);
     F[0] = f[0] + S * (fac - u[0]);
 #pragma unroll
     for (int b = 0; b < D; ++b) {
         const double us = fac * (b == a ? Sstar : K.v[b]);
         F[1 + b] = f[1 + b] + S * (us - u[1 + b]);
     }
-    const double es = fac * (K.e * K.ir + (Sstar - vn) * (Sstar + K.p / mK));
+    const double es = fac * (K.e * K.ir + (Sstar - vn) * (Sstar + K.p * fast_rcp(mK)));
     F[1 + D] = f[1 + D] + S * (es - K.e);
 }
 
@@ -383,8 +404,8 @@ __device__ __forceinline__ void wavespeed_points(const double *RA, double gamma,
         double v2 = 0.0;
 #pragma unroll
         for (int b = 0; b < D; ++b) v2 = fma(q.v[b], q.v[b], v2);
-        const double cs = sqrt(gamma * q.p * q.ir);
-        const double vm = sqrt(v2);
+        const double cs = fast_sqrt(gamma * q.p * q.ir);
+        const double vm = fast_sqrt(v2);
         cmax = (cs > cmax) ? cs : cmax;   // NaN-safe: NaN never becomes the maximum
         vmax = (vm > vmax) ? vm : vmax;
     }
@@ -392,26 +413,37 @@ __device__ __forceinline__ void wavespeed_points(const double *RA, double gamma,
     block_max2<NT>(cmax, vmax, red, maxbits, tid);
 }
 
+// address of row `row` (compile-time multiple after unrolling) of a [row][cell] global array: one IMAD.WIDE
+__device__ __forceinline__ const double *row_ptr(const double *base, unsigned row, unsigned ncells) {
+    return base + (unsigned long long)row * ncells;
+}
+__device__ __forceinline__ double *row_ptr(double *base, unsigned row, unsigned ncells) {
+    return base + (unsigned long long)row * ncells;
+}
+
 // Own modes of the block's cells, global [r = mode*V + v][cell] -> shared [v][mode][cell].  Thread `tid` keeps
-// cell tid % C; its loads are issued in batches of up to 12 before the first store (one DRAM round trip per batch).
+// cell tid % C and the modes g, g+G, ... (g = tid / C, G = NT / C) of every variable; its loads are issued in
+// batches of up to 12 before the first store (one DRAM round trip per batch).
 template <int V, int Np, int C, int NT, class L>
 __device__ __forceinline__ void load_own_modes(const double *__restrict__ w, int ncells, int cg, double *RA, int tid) {
-    constexpr int NR = (V * Np * C + NT - 1) / NT;
-    constexpr int RB = NR < 12 ? NR : 12;
-    const int cl = tid % C;
+    constexpr int G = NT / C;
+    constexpr int NK = (Np + G - 1) / G;
+    constexpr int KB = (12 / V) < 1 ? 1 : (12 / V);          // k-steps per batch
+    const int cl = tid % C, g = tid / C;
+    const double *base = w + (size_t)(g * V) * ncells + cg;
 #pragma unroll
-    for (int k0 = 0; k0 < NR; k0 += RB) {
-        double t[RB];
+    for (int k0 = 0; k0 < NK; k0 += KB) {
+        double t[KB][V];
 #pragma unroll
-        for (int j = 0; j < RB; ++j) {
-            const int r = tid / C + (k0 + j) * (NT / C);
-            if (k0 + j < NR && r < V * Np) t[j] = __ldg(w + (size_t)r * ncells + cg);
-        }
+        for (int kk = 0; kk < KB; ++kk)
 #pragma unroll
-        for (int j = 0; j < RB; ++j) {
-            const int r = tid / C + (k0 + j) * (NT / C);
-            if (k0 + j < NR && r < V * Np) RA[L::at2(r % V, r / V) * C + cl] = t[j];
-        }
+            for (int v = 0; v < V; ++v)
+                if (k0 + kk < NK && g + (k0 + kk) * G < Np) t[kk][v] = __ldg(row_ptr(base, (k0 + kk) * G * V + v, ncells));
+#pragma unroll
+        for (int kk = 0; kk < KB; ++kk)
+#pragma unroll
+            for (int v = 0; v < V; ++v)
+                if (k0 + kk < NK && g + (k0 + kk) * G < Np) RA[L::at2(v, g + (k0 + kk) * G) * C + cl] = t[kk][v];
     }
 }
 
@@ -587,8 +619,8 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA
                 }
                 if (AV) {
                     const double al = RX[LF::at2(oUT + Vc, k) * C + cell];
-                    const double cst = sqrt(p.gamma * qt.p * qt.ir);
-                    const double eps = fmin(fmax(al, 0.0), p.alpha_max) * cst * p.h / (double)M;   // Eq. 46, A12
+                    const double cst = fast_sqrt(p.gamma * qt.p * qt.ir);
+                    const double eps = fmin(fmax(al, 0.0), p.alpha_max) * cst * (p.h / (double)M);   // Eq. 46, A12
 #pragma unroll
                     for (int v = 0; v < Vc; ++v) Fh[v] -= eps * g[A][v];
                 }
@@ -718,20 +750,22 @@ __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(co
     double Fp[D][NLIFT], Fm[D][NLIFT];
 #pragma unroll
     for (int a = 0; a < D; ++a) {
-        const double *fl = p.flux + (size_t)a * NFL * p.ncells;
+        const double *fp = p.flux + (size_t)(tid / C) * p.ncells + cg;
+        const double *fm = p.flux + (size_t)(tid / C) * p.ncells + nbm[a];
 #pragma unroll
         for (int k = 0; k < NLIFT; ++k) {
-            const int r = tid / C + k * (NT / C);
-            if (r < NFL) {
-                Fp[a][k] = __ldg(fl + (size_t)r * p.ncells + cg);
-                Fm[a][k] = __ldg(fl + (size_t)r * p.ncells + nbm[a]);
+            if (tid / C + k * (NT / C) < NFL) {
+                Fp[a][k] = __ldg(row_ptr(fp, a * NFL + k * (NT / C), p.ncells));
+                Fm[a][k] = __ldg(row_ptr(fm, a * NFL + k * (NT / C), p.ncells));
             }
         }
     }
     if (!p.rhs_only && cl % 4 == 0) {
         // u^n is needed only by the stage combine at the very end: start it towards L2 now
-        for (int r = tid / C; r < V * Np; r += NT / C)
-            asm volatile("prefetch.global.L2 [%0];" ::"l"(p.w_n + (size_t)r * p.ncells + cg));
+        const double *wn = p.w_n + (size_t)(tid / C) * p.ncells + cg;
+#pragma unroll 4
+        for (int k = 0; tid / C + k * (NT / C) < V * Np; ++k)
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(row_ptr(wn, k * (NT / C), p.ncells)));
     }
     if (AV && tid < C) {
         // wiggle source of Eq. 45 from the previous step's sensor (readings A14, A15)
@@ -800,6 +834,7 @@ __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(co
     {
         // V3: point-wise fluxes G_a = f_a - F_NS,a - eps d_a u (Eq. 24; 315 Eq. 38), alpha source
         bool bad = false;
+        const double decay = (double)M / (p.f_tau * p.h);      // 1/tau = (n+1) c_s / (f_tau h), Eq. 44
         for (int it = tid; it < Np * C; it += NT) {
             const int cell = it % C;
             const int j = it / C;
@@ -821,10 +856,10 @@ __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(co
             }
             if (AV) {
                 const double al = RA[L::at2(Vc, j) * C + cell];
-                const double cs = sqrt(p.gamma * q.p * q.ir);
-                eps = fmin(fmax(al, 0.0), p.alpha_max) * cs * p.h / (double)M;        // Eq. 46, A17
+                const double cs = fast_sqrt(p.gamma * q.p * q.ir);
+                eps = fmin(fmax(al, 0.0), p.alpha_max) * cs * (p.h / (double)M);        // Eq. 46, A17
                 // Eq. 43-45: shock source + wiggle source - decay; stored pre-scaled by h/2 for the projection
-                const double src = p.f_v * fmax(0.0, -divv) + Wk[cell] - al * ((double)M * cs / (p.f_tau * p.h));
+                const double src = p.f_v * fmax(0.0, -divv) + Wk[cell] - al * (cs * decay);
                 RA[L::at2(Vc, j) * C + cell] = 0.5 * p.h * src;
             }
 #pragma unroll
@@ -919,40 +954,43 @@ __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(co
     const double cdt = p.rhs_only ? 1.0 : p.rk_c * p.scal[0];
     double sA = 0.0, sB = 0.0, dA = 0.0, dB = 0.0;
     {
-        constexpr int NR = (V * Np * C + NT - 1) / NT;
-        constexpr int RB = NR < 6 ? NR : 6;
+        // same ownership as load_own_modes: modes g, g+G, ... of every variable of cell cl
+        constexpr int G = NT / C;
+        constexpr int NK = (Np + G - 1) / G;
+        const int g = tid / C;
         const bool active = cell0 + cl < p.ncells;
         const bool need_n = !p.rhs_only, need_p = !p.rhs_only && p.rk_b != 0.0;
+        const double *bn = p.w_n + (size_t)(g * V) * p.ncells + cg;
+        const double *bp = p.w_prev + (size_t)(g * V) * p.ncells + cg;
+        double *bo = p.w_out + (size_t)(g * V) * p.ncells + cg;
 #pragma unroll
-        for (int k0 = 0; k0 < NR; k0 += RB) {
-            double wn[RB], wp[RB];
+        for (int k = 0; k < NK; ++k) {
+            const int mode = g + k * G;
+            double wn[V], wp[V];
 #pragma unroll
-            for (int j = 0; j < RB; ++j) {
-                const int r = tid / C + (k0 + j) * (NT / C);
-                wn[j] = wp[j] = 0.0;
-                if (k0 + j < NR && r < V * Np) {
-                    if (need_n) wn[j] = __ldg(p.w_n + (size_t)r * p.ncells + cg);
-                    if (need_p) wp[j] = __ldg(p.w_prev + (size_t)r * p.ncells + cg);
+            for (int v = 0; v < V; ++v) {
+                wn[v] = wp[v] = 0.0;
+                if (mode < Np) {
+                    if (need_n) wn[v] = __ldg(row_ptr(bn, k * G * V + v, p.ncells));
+                    if (need_p) wp[v] = __ldg(row_ptr(bp, k * G * V + v, p.ncells));
                 }
             }
+            int rem = mode, top = 0;
 #pragma unroll
-            for (int j = 0; j < RB; ++j) {
-                const int r = tid / C + (k0 + j) * (NT / C);
-                if (k0 + j < NR && r < V * Np) {
-                    const int mode = r / V, v = r % V;
+            for (int a = 0; a < D; ++a) {
+                top |= (rem % M == M - 1);
+                rem /= M;
+            }
+#pragma unroll
+            for (int v = 0; v < V; ++v) {
+                if (mode < Np) {
                     const double Ld = ACC[L::at2(v, mode) * C + cl];
                     double wnew = Ld;
-                    if (!p.rhs_only) wnew = fma(cdt, Ld, fma(p.rk_b, wp[j], p.rk_a * wn[j]));
-                    if (active) p.w_out[(size_t)r * p.ncells + cg] = wnew;
+                    if (!p.rhs_only) wnew = fma(cdt, Ld, fma(p.rk_b, wp[v], p.rk_a * wn[v]));
+                    if (active) *row_ptr(bo, k * G * V + v, p.ncells) = wnew;
                     if (p.do_wavespeed) RA[L::at2(v, mode) * C + cl] = wnew;
                     if (AV && p.do_sensor && v == 0) {
-                        int rem = mode, top = 0;
-#pragma unroll
-                        for (int a = 0; a < D; ++a) {
-                            top |= (rem % M == M - 1);
-                            rem /= M;
-                        }
-                        const double w = wn[j];
+                        const double w = wn[v];
                         sB = fma(w, w, sB);
                         dB = fma(w, Ld, dB);
                         if (top && M > 1) {

@@ -123,6 +123,12 @@ int dg_get_time(dg_solver *s, double *t, double *last_dt);
  * per block, dynamic shared memory bytes per block, number of blocks.  Any pointer may be NULL. */
 int dg_kernel_info(dg_solver *s, int *cells_per_block, int *threads, int *smem_bytes, int *blocks);
 
+/* Device time of the two kernels of one RK stage, measured with CUDA events on the solver's stream around each
+ * launch: `reps` evaluations of dw/dt = L(w) of the current state (the state is not advanced), averages in
+ * milliseconds.  face_ms / stage_ms are HOST pointers (either may be NULL).  Used by bench.py for the per-kernel
+ * roofline; the evaluation is the `dg_eval_rhs` path (no stage combine reads of u^n, no wave-speed pass). */
+int dg_profile_stage(dg_solver *s, int reps, double *face_ms, double *stage_ms);
+
 /* Number of kernel launches issued by this solver since dg_init (graph replays count their nodes). */
 int dg_launch_count(dg_solver *s, long long *count);
 

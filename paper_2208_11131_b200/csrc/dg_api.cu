@@ -530,6 +530,43 @@ int dg_eval_rhs(dg_solver *s, double *out, size_t count, double *alpha_out, size
     return check_flag(s);
 }
 
+int dg_profile_stage(dg_solver *s, int reps, double *face_ms, double *stage_ms) {
+    if (!s) return fail(DG_EINVAL, "solver is NULL");
+    if (reps < 1) return fail(DG_EINVAL, "reps must be >= 1");
+    DgStageArgs a;
+    fill_args(s, &a);
+    a.w_prev = s->W0;
+    a.w_n = s->W0;
+    a.w_out = s->WA;
+    a.rhs_only = 1;
+    cudaEvent_t ev[3];
+    for (int i = 0; i < 3; ++i) CU(cudaEventCreate(&ev[i]));
+    double tf = 0.0, ts = 0.0;
+    int rc = DG_OK;
+    for (int k = 0; k < reps + 1 && rc == DG_OK; ++k) {   // first pass is a warm-up
+        cudaError_t e = cudaEventRecord(ev[0], s->stream);
+        if (e == cudaSuccess) e = s->fn.launch(s->visc, s->av, &a, s->stream, 2);
+        if (e == cudaSuccess) e = cudaEventRecord(ev[1], s->stream);
+        if (e == cudaSuccess) e = s->fn.launch(s->visc, s->av, &a, s->stream, 3);
+        if (e == cudaSuccess) e = cudaEventRecord(ev[2], s->stream);
+        if (e == cudaSuccess) e = cudaEventSynchronize(ev[2]);
+        float f = 0.f, g = 0.f;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&f, ev[0], ev[1]);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&g, ev[1], ev[2]);
+        if (e != cudaSuccess) rc = fail(DG_ECUDA, "dg_profile_stage: %s", cudaGetErrorString(e));
+        s->launches += 2;
+        if (k > 0) {
+            tf += f;
+            ts += g;
+        }
+    }
+    for (int i = 0; i < 3; ++i) cudaEventDestroy(ev[i]);
+    if (rc) return rc;
+    if (face_ms) *face_ms = tf / reps;
+    if (stage_ms) *stage_ms = ts / reps;
+    return check_flag(s);
+}
+
 int dg_get_time(dg_solver *s, double *t, double *last_dt) {
     if (!s) return fail(DG_EINVAL, "solver is NULL");
     double v[2];

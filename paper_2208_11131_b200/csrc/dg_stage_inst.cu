@@ -28,16 +28,19 @@ template <bool VISC, bool AV>
 cudaError_t launch(const DgStageArgs &a, cudaStream_t st, int wavespeed_only) {
     using K = dgk::Cfg<DG_DIM, DG_M, VISC, AV>;
     const int blocks = (a.ncells + K::C - 1) / K::C;
-    if (wavespeed_only) {
+    // wavespeed_only: 0 = face + stage kernels, 1 = wave-speed kernel, 2 = face kernel only, 3 = stage kernel only
+    if (wavespeed_only == 1) {
         dgk::dg_wavespeed_kernel<DG_DIM, DG_M, VISC, AV><<<blocks, K::NT, K::kSmemBytes, st>>>(a);
-    } else {
+        return cudaGetLastError();
+    }
+    if (wavespeed_only != 3) {
         using FK = dgk::FaceCfg<DG_DIM, DG_M, VISC, AV>;
         const int fblocks = (a.ncells + FK::C - 1) / FK::C;
         dgk::dg_face_kernel<DG_DIM, DG_M, VISC, AV><<<fblocks, FK::NT, FK::kSmemBytes, st>>>(a);
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;
-        dgk::dg_stage_kernel<DG_DIM, DG_M, VISC, AV><<<blocks, K::NT, K::kSmemBytes, st>>>(a);
     }
+    if (wavespeed_only != 2) dgk::dg_stage_kernel<DG_DIM, DG_M, VISC, AV><<<blocks, K::NT, K::kSmemBytes, st>>>(a);
     return cudaGetLastError();
 }
 

@@ -57,6 +57,7 @@ SYMBOLS = {
     "dg_eval_rhs": (C.c_int, [_P, _P, C.c_size_t, _P, C.c_size_t]),
     "dg_get_time": (C.c_int, [_P, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
     "dg_kernel_info": (C.c_int, [_P, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int)]),
+    "dg_profile_stage": (C.c_int, [_P, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
     "dg_launch_count": (C.c_int, [_P, C.POINTER(C.c_longlong)]),
     "dg_measure_fp64_peak": (C.c_int, [C.c_int, C.POINTER(C.c_double), _P]),
     "dg_free": (C.c_int, [_P]),
@@ -204,6 +205,12 @@ class Solver:
         c, nt, sm, nb = C.c_int(), C.c_int(), C.c_int(), C.c_int()
         _check(self._lib.dg_kernel_info(self._h, C.byref(c), C.byref(nt), C.byref(sm), C.byref(nb)))
         return dict(cells_per_block=c.value, threads=nt.value, smem_bytes=sm.value, blocks=nb.value)
+
+    def profile_stage(self, reps=3):
+        """(face_ms, stage_ms): device time of the two kernels of one RK stage (CUDA events on the solver stream)."""
+        f, g = C.c_double(), C.c_double()
+        _check(self._lib.dg_profile_stage(self._h, reps, C.byref(f), C.byref(g)))
+        return f.value, g.value
 
     def launch_count(self):
         n = C.c_longlong()

@@ -34,18 +34,13 @@ def pointwise_flops(d: int, visc: bool, av: bool):
     return vol, face
 
 
-def stage_flops_per_cell(d: int, m: int, visc: bool, av: bool) -> float:
+def face_kernel_flops_per_cell(d: int, m: int, visc: bool, av: bool) -> float:
+    """dg_face_kernel: d faces per cell, each evaluated once (traces, recovery, flux, transverse projection)."""
     Vc = d + 2
     V = Vc + (1 if av else 0)
     grad = visc or av
-    Np, Nf = m ** d, m ** (d - 1)
-    s = 2.0 * m                                   # flops per output value of a 1D sweep
-    fl = V * d * Np * s                           # expansion (Eq. 21)
-    fl += Vc * d * Np * s                         # weak-form derivative, N = sum_a S_a G_a
-    fl += V * d * Np * s                          # projection on the modes
-    if grad:
-        fl += Vc * d * Np * s                     # gradients at the Gauss points
-    # one face per axis per cell
+    Nf = m ** (d - 1)
+    s = 2.0 * m
     per_face = 2 * Vc * Nf * s                    # two one-sided traces
     nqe = 2 * Vc
     if grad:
@@ -54,11 +49,45 @@ def stage_flops_per_cell(d: int, m: int, visc: bool, av: bool) -> float:
         nqe = 3 * Vc + V
     per_face += nqe * (d - 1) * Nf * s            # transverse modal -> nodal
     per_face += Vc * (d - 1) * Nf * s             # projection of the flux
-    per_face += 2 * Vc * Nf * m * 2               # lift into both cells
-    cv, cf = pointwise_flops(d, visc, av)
-    fl += d * (per_face + Nf * cf) + Np * cv
+    _, cf = pointwise_flops(d, visc, av)
+    return d * (per_face + Nf * cf)
+
+
+def stage_kernel_flops_per_cell(d: int, m: int, visc: bool, av: bool) -> float:
+    """dg_stage_kernel: lift of the 2d faces, volume term, stage combine."""
+    Vc = d + 2
+    V = Vc + (1 if av else 0)
+    grad = visc or av
+    Np, Nf = m ** d, m ** (d - 1)
+    s = 2.0 * m
+    fl = V * d * Np * s                           # expansion (Eq. 21)
+    fl += Vc * d * Np * s                         # weak-form derivative, N = sum_a S_a G_a
+    fl += V * d * Np * s                          # projection on the modes
+    if grad:
+        fl += Vc * d * Np * s                     # gradients at the Gauss points
+    cv, _ = pointwise_flops(d, visc, av)
+    fl += Np * cv
+    fl += d * 2 * Vc * Nf * m * 2                 # lift of each face into both cells (d faces per cell)
     fl += 3 * V * Np                              # stage combine (mean over the stages is ~2.7 fma)
     return fl
+
+
+def stage_flops_per_cell(d: int, m: int, visc: bool, av: bool) -> float:
+    """Whole RK stage (both kernels)."""
+    return face_kernel_flops_per_cell(d, m, visc, av) + stage_kernel_flops_per_cell(d, m, visc, av)
+
+
+def kernel_bytes_per_cell(d: int, m: int, av: bool, rk_stages: int = 3):
+    """Compulsory HBM bytes per cell of the two kernels of one stage (halo / neighbour re-reads are not counted):
+    face kernel reads the state once and writes the projected face fluxes; stage kernel reads the stage input, u^n
+    on all but the first stage, its own face fluxes, and writes the stage output."""
+    Vc = d + 2
+    V = Vc + (1 if av else 0)
+    state = 8.0 * V * m ** d
+    flux = 8.0 * d * Vc * m ** (d - 1)
+    face = state + flux
+    stage = state + state * (rk_stages - 1) / rk_stages + flux + state
+    return face, stage
 
 
 def stage_bytes_per_cell(d: int, m: int, av: bool, rk_stages: int = 3) -> float:

@@ -60,8 +60,9 @@ def test_no_cpu_fallback_and_argument_validation():
 
 
 def test_workspace_size_matches_the_memory_model():
-    """3 state buffers (u^n and two stage buffers) of V*M*Ncells doubles: the paper's Eq. 59-62 book-keeping
-     with f_t = 3 minus the dw/dt array the fused kernel never stores."""
+    """3 state buffers (u^n and two stage buffers) of V*M*Ncells doubles -- the paper's Eq. 59-62 book-keeping
+     with f_t = 3 minus the dw/dt array the stage kernel never stores -- plus the projected
+    face fluxes (d * Vc * m^(d-1) doubles per cell) and the two sensor scalars per cell."""
     import ctypes as C
     from paper_2208_11131_b200 import dg
     lib = dg.load_library()
@@ -74,7 +75,8 @@ def test_workspace_size_matches_the_memory_model():
     opt = dg.default_options(av_enable=1)
     assert lib.dg_workspace_bytes(C.byref(mesh), 4, C.byref(opt), C.byref(need)) == 0
     state = 6 * 64 * 16 ** 3 * 8
-    assert 3 * state <= need.value <= 3 * state + 4 * 16 ** 3 * 8 + 4096
+    flux = 3 * 5 * 16 * 16 ** 3 * 8
+    assert 3 * state + flux <= need.value <= 3 * state + flux + 4 * 16 ** 3 * 8 + 4096
 
 
 def test_roofline_model():
@@ -83,6 +85,9 @@ def test_roofline_model():
     f = [rl.stage_flops_per_cell(3, m, False, False) for m in range(1, 9)]
     assert all(b > a for a, b in zip(f, f[1:]))
     assert rl.stage_flops_per_cell(3, 4, True, True) > rl.stage_flops_per_cell(3, 4, True, False) > f[3]
+    assert rl.stage_flops_per_cell(3, 4, True, True) == (rl.face_kernel_flops_per_cell(3, 4, True, True)
+                                                         + rl.stage_kernel_flops_per_cell(3, 4, True, True))
+    assert rl.kernel_bytes_per_cell(3, 4, True) == (3072 + 1920, 3072 * (1 + 2 / 3 + 1) + 1920)
     r = rl.roofline(3, 4, True, True, 128 ** 3, 10e-3, 6535.0, rl.NOMINAL_FP64_TFLOPS)
     assert r["bound"] == "alu" and 0 < r["alu_frac"] < 1 and abs(r["t_hbm_ms"] - 2.63) < 0.05
 

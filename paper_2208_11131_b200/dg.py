@@ -189,12 +189,18 @@ class Solver:
         _check(self._lib.dg_conserved_totals(self._h, C.byref(t)))
         return np.array(t[:self.Vc])
 
-    def eval_rhs(self, with_alpha=False):
-        out = np.empty(self.Vc * self.M * self.ncells)
-        al = np.empty(self.M * self.ncells) if with_alpha else None
-        _check(self._lib.dg_eval_rhs(self._h, out.ctypes.data, out.size, al.ctypes.data if with_alpha else None,
-                                     al.size if with_alpha else 0))
-        return (out, al) if with_alpha else out
+    def eval_rhs(self, with_alpha=False, out=None, alpha_out=None):
+        """dw/dt of the current state.  `out` / `alpha_out` may be numpy arrays or torch tensors (host or cuda)."""
+        if out is None:
+            out = np.empty(self.Vc * self.M * self.ncells)
+        if alpha_out is None and with_alpha:
+            alpha_out = np.empty(self.M * self.ncells)
+        po, no, _ = _buf(out)
+        pa, na = None, 0
+        if alpha_out is not None:
+            pa, na, _ = _buf(alpha_out)
+        _check(self._lib.dg_eval_rhs(self._h, po, no, pa, na))
+        return (out, alpha_out) if alpha_out is not None else out
 
     def get_time(self):
         t, dt = C.c_double(), C.c_double()

@@ -16,6 +16,15 @@ TOL_1 = 1e-12
 TOL_10 = 1e-9
 
 
+def _report(line):
+    """Measured differences are appended to gpurun_out/parity_report.txt (scratch; copied into profiles/ by hand)."""
+    import os
+    d = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out")
+    if os.path.isdir(d):
+        with open(os.path.join(d, "parity_report.txt"), "a") as f:
+            f.write(line + "\n")
+
+
 def _wl(d, ncell, n, phys, f_cfl=0.3):
     return wk.Workload("rand", d, tuple(ncell), 1.0 / ncell[0], n, 1.4 if d == 2 else 5.0 / 3.0,
                        nu=0.01 if "ns" in phys else 0.0, chi=0.02 if "ns" in phys else 0.0,
@@ -99,6 +108,8 @@ def test_step_parity(cfg, degree):
     g.step(9)
     e10 = parity_norm(g.get_state(), o.get_state(), wl)
     assert np.all(e10 <= TOL_10), ("10 steps", e10)
+    _report("%s degree %d mesh %s: 1 step %.3e, 10 steps %.3e" % (wl.name, wl.degree, "x".join(map(str, wl.ncell)),
+                                                                  np.max(e1), np.max(e10)))
     if wl.av:
         assert np.max(np.abs(g.get_alpha() - o.get_alpha())) <= TOL_10
     # conserved totals agree with the oracle's and with the initial ones
@@ -205,3 +216,74 @@ def test_device_pointer_io():
     out = torch.empty(w0.size, dtype=torch.float64, device="cuda")
     g.get_state(out)
     assert np.array_equal(out.cpu().numpy(), w0)
+
+
+# ---------------------------------------------------------------------------------------------------
+# full-size parity in the launch configuration bench.py times (BASELINE config 4: 128^3, degree 3, NS + AV):
+# dw/dt of sampled cells.  L(w) of a cell depends only on the cell and its 2d face neighbours, so a periodic
+# 3x3x3 oracle mesh holding the sampled cell's neighbourhood reproduces that cell's dw/dt exactly.
+# ---------------------------------------------------------------------------------------------------
+def _tiled_state(wl, block=16, seed=5):
+    """Seeded state on the full mesh without 10^9 random draws: a random smooth block tiled over the mesh plus a
+    smooth large-scale modulation of the cell means, so that no two neighbourhoods are alike."""
+    d, Vc, M = wl.dim, wl.dim + 2, wl.modes
+    w0, al = wk.random_smooth_modes(d, (block,) * d, wl.degree, wl.gamma, seed=seed, amp=0.03, nvar_extra=1)
+    reps = tuple(n // block for n in reversed(wl.ncell))
+    w = np.tile(w0.reshape((M * Vc,) + (block,) * d), (1,) + reps)
+    a = np.tile(al.reshape((M,) + (block,) * d), (1,) + reps)
+    idx = np.meshgrid(*[np.arange(n) / n for n in reversed(wl.ncell)], indexing="ij")
+    mod = 1.0 + 0.05 * np.sin(2 * np.pi * sum((k + 1) * x for k, x in enumerate(idx)))
+    w = w.reshape((M, Vc) + w.shape[1:])
+    w[0, 0] *= mod
+    w[0, Vc - 1] *= mod
+    return np.ascontiguousarray(w).ravel(), np.ascontiguousarray(a).ravel()
+
+
+def test_full_size_sampled_rhs_parity():
+    import torch
+    wl = wk.config(4)
+    assert wl.ncell == (128, 128, 128) and wl.degree == 3 and wl.av and wl.nu > 0
+    d, Vc, M, N = wl.dim, wl.dim + 2, wl.modes, wl.ncells
+    w, al = _tiled_state(wl)
+    g = make_gpu(wl)
+    g.set_state(w)
+    g.set_alpha(al)
+    info = g.kernel_info()
+    assert info["blocks"] * info["cells_per_block"] >= N
+    L_dev = torch.empty(Vc * M * N, dtype=torch.float64, device="cuda")
+    La_dev = torch.empty(M * N, dtype=torch.float64, device="cuda")
+    g.eval_rhs(out=L_dev, alpha_out=La_dev)
+    L_dev = L_dev.view(M, Vc, N)
+    La_dev = La_dev.view(M, N)
+    nx, ny, nz = wl.ncell
+    wv = w.reshape(M, Vc, nz, ny, nx)
+    av = al.reshape(M, nz, ny, nx)
+    samples = [(0, 0, 0), (127, 127, 127), (127, 0, 64), (5, 127, 0), (64, 64, 64), (17, 93, 2), (126, 1, 127),
+               (8, 15, 16), (31, 32, 33)]
+    from dataclasses import replace
+    sub = replace(wl, ncell=(3, 3, 3))                      # same h, gamma, nu, chi, AV options
+    worst = 0.0
+    for (ix, iy, iz) in samples:
+        zi = [(iz + k) % nz for k in (-1, 0, 1)]
+        yi = [(iy + k) % ny for k in (-1, 0, 1)]
+        xi = [(ix + k) % nx for k in (-1, 0, 1)]
+        o = make_oracle(sub)
+        o.set_state(np.ascontiguousarray(wv[:, :, zi][:, :, :, yi][:, :, :, :, xi]).ravel())
+        o.set_alpha(np.ascontiguousarray(av[:, zi][:, :, yi][:, :, :, xi]).ravel())
+        Lo = o.rhs(o.w)                                    # [cell, mode, var]
+        centre = (1 * 3 + 1) * 3 + 1
+        cell = (iz * ny + iy) * nx + ix
+        Lg = L_dev[:, :, cell].cpu().numpy()
+        Lag = La_dev[:, cell].cpu().numpy()
+        ref = Lo[centre, :, :Vc]
+        scale = np.max(np.abs(Lo[:, :, :Vc]), axis=(0, 1))
+        scale[1:1 + d] = np.max(scale[1:1 + d])
+        err = np.max(np.abs(Lg - ref) / scale)
+        worst = max(worst, err)
+        assert err < 5e-12, ((ix, iy, iz), err)
+        assert np.max(np.abs(Lag - Lo[centre, :, Vc])) <= 5e-12 * max(1.0, np.max(np.abs(Lo[:, :, Vc])))
+    # properties that hold at any size: conservation of the cell-mean rows of dw/dt (PAPER.md:104 Eq. 10 summed)
+    tot = L_dev[0].sum(dim=1).cpu().numpy()
+    mag = L_dev[0].abs().sum(dim=1).cpu().numpy()
+    assert np.all(np.abs(tot) <= 1e-12 * mag), (tot, mag)
+    _report("full-size cfg4 128^3 sampled dw/dt: worst relative difference %.3e over %d cells" % (worst, len(samples)))

@@ -65,8 +65,8 @@ struct Cfg {
     static constexpr int RX = D * Vc * Np;                         // gradients -> fluxes (in place)
     static constexpr int FP = 2 * V * Np + RX;                     // doubles per cell
     static constexpr int NT = DG_STAGE_NT;
-    // W^K per cell, wave-speed reduction scratch, partial sensor sums
-    static constexpr int extra_doubles(int c) { return c + 2 * (NT / 32) + (AV ? 4 * (NT / 32) * c : 0); }
+    // W^K per cell, wave-speed reduction scratch, partial sensor sums, one mbarrier
+    static constexpr int extra_doubles(int c) { return c + 2 * (NT / 32) + (AV ? 4 * (NT / 32) * c : 0) + 2; }
     static constexpr int pick_c() {
         int c = 32;
         while (c > 1 && (c * FP + extra_doubles(c)) * 8 > kSmemBudget) c >>= 1;
@@ -421,6 +421,51 @@ __device__ __forceinline__ double *row_ptr(double *base, unsigned row, unsigned 
     return base + (unsigned long long)row * ncells;
 }
 
+// ---- bulk asynchronous copies (TMA engine, 1D): global -> shared, completion on an mbarrier ----
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(void *bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(void *bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(void *bar, unsigned parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned bytes, void *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+// Own modes of a FULL tile (C cells, 16-byte aligned rows) by bulk copies: one C*8-byte row segment per request,
+// global [r = mode*V + v][cell] -> shared [v][mode][cell]; no registers, no LSU queue slots.  Thread 0 must have
+// initialised `bar` (count 1) before a __syncthreads(); returns after the data has landed.
+template <int V, int Np, int C, int NT, class L>
+__device__ __forceinline__ void issue_own_modes_bulk(const double *w, int ncells, int cell0, double *RA, void *bar,
+                                                     int tid) {
+    if (tid == 0) mbar_expect_tx(bar, (unsigned)(V * Np * C * 8));
+    for (int r = tid; r < V * Np; r += NT)
+        bulk_g2s(RA + L::at2(r % V, r / V) * C, w + (size_t)r * ncells + cell0, C * 8, bar);
+}
+// a tile qualifies for bulk copies when it is full and every row segment is 16-byte aligned
+template <int C>
+__device__ __forceinline__ bool bulk_ok(int cell0, int ncells) {
+    return (C % 2 == 0) && (cell0 + C <= ncells) && ((ncells & 1) == 0);
+}
+
 // Own modes of the block's cells, global [r = mode*V + v][cell] -> shared [v][mode][cell].  Thread `tid` keeps
 // cell tid % C and the modes g, g+G, ... (g = tid / C, G = NT / C) of every variable; its loads are issued in
 // batches of up to 12 before the first store (one DRAM round trip per batch).
@@ -465,7 +510,7 @@ struct FaceCfg {
         return c;
     }
     static constexpr int C = pick_c();
-    static constexpr int kSmemBytes = C * FP * 8 + D * C * 4;
+    static constexpr int kSmemBytes = C * FP * 8 + ((D * C + 1) / 2) * 8 + 16;   // + nbr[D*C] + mbarrier
     static_assert(kSmemBytes <= kSmemMax, "face kernel: per-cell footprint exceeds shared memory");
     static constexpr bool SWZ = use_swizzle(M, C);
     using LV = Lay<M * M, K::Np, SWZ>;          // own modes (volume array)
@@ -686,12 +731,19 @@ __global__ void __launch_bounds__(DG_FACE_NT, DG_FACE_MINB) dg_face_kernel(const
     using K = Cfg<D, M, VISC, AV>;
     using FK = FaceCfg<D, M, VISC, AV>;
     constexpr int C = FK::C, NT = FK::NT, V = K::V, Np = K::Np;
-    extern __shared__ double smem[];
+    extern __shared__ __align__(128) double smem[];
     double *RA = smem;
     double *RX = RA + V * Np * C;
     int *nbr = reinterpret_cast<int *>(RX + K::NQ * K::Nf * C);
+    double *bar = RX + K::NQ * K::Nf * C + (D * C + 1) / 2;   // mbarrier of the bulk copies, after nbr[D*C]
     const int tid = threadIdx.x;
     const int cell0 = blockIdx.x * C;
+    const bool bulk = bulk_ok<C>(cell0, p.ncells);
+    if (bulk) {
+        if (tid == 0) mbar_init(bar, 1);
+        __syncthreads();
+        issue_own_modes_bulk<V, Np, C, NT, typename FK::LV>(p.w_prev, p.ncells, cell0, RA, bar, tid);
+    }
     if (tid < C) {
         const int c = min(cell0 + tid, p.ncells - 1);
         const int ix = c % p.nx;
@@ -704,7 +756,10 @@ __global__ void __launch_bounds__(DG_FACE_NT, DG_FACE_MINB) dg_face_kernel(const
             nbr[(D - 1) * C + tid] = c + ((iz == p.nz - 1) ? -(p.nz - 1) * pl : pl);
         }
     }
-    load_own_modes<V, Np, C, NT, typename FK::LV>(p.w_prev, p.ncells, min(cell0 + tid % C, p.ncells - 1), RA, tid);
+    if (bulk)
+        mbar_wait(bar, 0);
+    else
+        load_own_modes<V, Np, C, NT, typename FK::LV>(p.w_prev, p.ncells, min(cell0 + tid % C, p.ncells - 1), RA, tid);
     __syncthreads();
     face_axis<D, M, VISC, AV, 0>(p, RA, RX, nbr, cell0, tid);
     face_axis<D, M, VISC, AV, 1>(p, RA, RX, nbr, cell0, tid);
@@ -721,15 +776,23 @@ __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(co
     constexpr bool GRAD = K::GRAD, BLK = K::BLK;
     using L = Lay<M * M, Np, use_swizzle(M, C)>;
     constexpr int NTILE = Np / (M * M);          // m x m tiles per slot (m in 3D, 1 in 2D)
-    extern __shared__ double smem[];
+    extern __shared__ __align__(128) double smem[];
     double *RA = smem;
     double *RX = RA + V * Np * C;
     double *ACC = RX + K::RX * C;
     double *Wk = ACC + V * Np * C;
     double *red = Wk + C;
     double *sens = red + 2 * (NT / 32);           // [4][NT/32][C] partial sensor sums (AV only)
+    double *bar = sens + (AV ? 4 * (NT / 32) * C : 0);   // mbarrier of the bulk copies
     const int tid = threadIdx.x;
     const int cell0 = blockIdx.x * C;
+    // own modes of a full tile travel global -> RA as bulk asynchronous copies (one request per row segment)
+    const bool bulk = bulk_ok<C>(cell0, p.ncells);
+    if (bulk) {
+        if (tid == 0) mbar_init(bar, 1);
+        __syncthreads();
+        issue_own_modes_bulk<V, Np, C, NT, L>(p.w_prev, p.ncells, cell0, RA, bar, tid);
+    }
 
     // every thread works on one fixed cell of the block (NT is a multiple of C)
     static_assert(NT % C == 0, "threads per block must be a multiple of cells per block");
@@ -774,8 +837,11 @@ __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(co
         Wk[tid] = (S > p.s_onset) ? p.f_w * fmax(0.0, G) : 0.0;
     }
     // own modes -> RA, zero ACC
-    load_own_modes<V, Np, C, NT, L>(p.w_prev, p.ncells, cg, RA, tid);   // global slot order: r = mode*V + v
     for (int r = tid / C; r < V * Np; r += NT / C) ACC[r * C + cl] = 0.0;
+    if (bulk)
+        mbar_wait(bar, 0);
+    else
+        load_own_modes<V, Np, C, NT, L>(p.w_prev, p.ncells, cg, RA, tid);   // global slot order: r = mode*V + v
     __syncthreads();
 
     // ---- surface term: lift the face fluxes of dg_face_kernel along each normal (Eq. 20, readings A3/A4) ----
@@ -1048,7 +1114,7 @@ __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_wavespeed_kerne
     using K = Cfg<D, M, VISC, AV>;
     constexpr int C = K::C, NT = K::NT, V = K::V, Vc = K::Vc, Np = K::Np;
     using L = Lay<M * M, Np, use_swizzle(M, C)>;
-    extern __shared__ double smem[];
+    extern __shared__ __align__(128) double smem[];
     double *RA = smem;
     double *red = RA + V * Np * C + K::RX * C + V * Np * C + C;
     const int tid = threadIdx.x;

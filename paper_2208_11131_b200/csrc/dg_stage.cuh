@@ -539,15 +539,22 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA
         const int cell = tid % C;
         const int nc = nbr[A * C + cell];
         double nb[NIT][M];
+        // the upper x neighbour of every cell but the last one of the tile is the next cell of the tile itself
+        const bool from_tile = (A == 0) && (cell < C - 1) && (cell0 + cell + 1 < p.ncells) && (nc == cell0 + cell + 1);
 #pragma unroll
         for (int k = 0; k < NIT; ++k) {
             const int r = tid / C + k * (NT / C);          // v*Nf + lt
             if (r < V * Nf) {
                 const int base = pencil_base<M, SA>(r % Nf);
                 const int v = r / Nf;
+                if (from_tile) {
 #pragma unroll
-                for (int l = 0; l < M; ++l)
-                    nb[k][l] = __ldg(p.w_prev + (size_t)((base + l * SA) * V + v) * p.ncells + nc);
+                    for (int l = 0; l < M; ++l) nb[k][l] = RA[LV::at2(v, base + l * SA) * C + cell + 1];
+                } else {
+#pragma unroll
+                    for (int l = 0; l < M; ++l)
+                        nb[k][l] = __ldg(p.w_prev + (size_t)((base + l * SA) * V + v) * p.ncells + nc);
+                }
             }
         }
 #pragma unroll

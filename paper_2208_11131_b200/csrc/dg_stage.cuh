@@ -85,20 +85,33 @@ struct Cfg {
 // the lanes of a warp walk over planes / slots (strides that are multiples of 16 doubles).  For even m the two rows
 // of a pair are exchanged according to the parity of (plane index + slot index), which makes every access pattern
 // of the kernels below conflict-free (pencils along any axis, m x m tiles, point-wise, row-wise I/O).
-template <int PL, int NPTS, bool SWZ>
+template <int PL, int NPTS, bool SWZ, int ROTM = 0>
 struct Lay {
+    // ROTM = m (pencil sweeps with few cells per block, m even): the x index of every row of m points is rotated by
+    // the row's y index, x' = (x + y) mod m.  Pencils along x of different rows then start in different banks, and
+    // every other access pattern still touches the same set of addresses per row.
+    static __device__ __forceinline__ int rot(int j) {
+        if (ROTM > 0) {
+            const int row = j / ROTM;
+            int x = j - row * ROTM + row % ROTM;
+            if (x >= ROTM) x -= ROTM;
+            return row * ROTM + x;
+        }
+        return j;
+    }
     static __device__ __forceinline__ int at(int P) {
         if (SWZ) {
             const int par = P / PL + (NPTS > PL ? P / NPTS : 0);
             return P ^ (par & 1);
         }
+        if (ROTM > 0) return (P / NPTS) * NPTS + rot(P % NPTS);
         return P;
     }
     // same as at(slot*NPTS + j); with `slot` a compile-time constant after unrolling this needs one runtime XOR per j
     // (NPTS / PL is even or 1 whenever SWZ is on)
     static __device__ __forceinline__ int at2(int slot, int j) {
         if (SWZ) return slot * NPTS + (j ^ ((j / PL + slot) & 1));
-        return slot * NPTS + j;
+        return slot * NPTS + rot(j);
     }
     // parity of tile g (PL points per tile): rows q and q^1 of the tile are exchanged when it is 1
     static __device__ __forceinline__ int tile_par(int g) {
@@ -106,6 +119,8 @@ struct Lay {
     }
 };
 __host__ __device__ constexpr bool use_swizzle(int M, int C) { return (M % 2 == 0) && (C == 8); }
+// rotation for the pencil-sweep path (m x m tiles not in registers), few cells per block, even m
+__host__ __device__ constexpr int use_rot(int M, int C, bool BLK) { return (!BLK && C < 8 && M % 2 == 0 && M > 1) ? M : 0; }
 
 template <int SEL>
 __device__ __forceinline__ double mat(int idx) {
@@ -513,8 +528,8 @@ struct FaceCfg {
     static constexpr int kSmemBytes = C * FP * 8 + ((D * C + 1) / 2) * 8 + 16;   // + nbr[D*C] + mbarrier
     static_assert(kSmemBytes <= kSmemMax, "face kernel: per-cell footprint exceeds shared memory");
     static constexpr bool SWZ = use_swizzle(M, C);
-    using LV = Lay<M * M, K::Np, SWZ>;          // own modes (volume array)
-    using LF = Lay<K::Nf, K::Nf, SWZ>;          // face arrays: one tile (3D) / one pencil (2D) per slot
+    using LV = Lay<M * M, K::Np, SWZ, use_rot(M, C, K::BLK)>;   // own modes (volume array)
+    using LF = Lay<K::Nf, K::Nf, SWZ, (D == 3 ? use_rot(M, C, K::BLK) : 0)>;          // face arrays: one tile (3D) / one pencil (2D) per slot
 };
 
 template <int D, int M, bool VISC, bool AV, int A>
@@ -781,7 +796,7 @@ __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(co
     using K = Cfg<D, M, VISC, AV>;
     constexpr int C = K::C, NT = K::NT, V = K::V, Vc = K::Vc, Np = K::Np;
     constexpr bool GRAD = K::GRAD, BLK = K::BLK;
-    using L = Lay<M * M, Np, use_swizzle(M, C)>;
+    using L = Lay<M * M, Np, use_swizzle(M, C), use_rot(M, C, K::BLK)>;
     constexpr int NTILE = Np / (M * M);          // m x m tiles per slot (m in 3D, 1 in 2D)
     extern __shared__ __align__(128) double smem[];
     double *RA = smem;
@@ -1120,7 +1135,7 @@ template <int D, int M, bool VISC, bool AV>
 __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_wavespeed_kernel(const DgStageArgs p) {
     using K = Cfg<D, M, VISC, AV>;
     constexpr int C = K::C, NT = K::NT, V = K::V, Vc = K::Vc, Np = K::Np;
-    using L = Lay<M * M, Np, use_swizzle(M, C)>;
+    using L = Lay<M * M, Np, use_swizzle(M, C), use_rot(M, C, K::BLK)>;
     extern __shared__ __align__(128) double smem[];
     double *RA = smem;
     double *red = RA + V * Np * C + K::RX * C + V * Np * C + C;

@@ -91,11 +91,12 @@ struct Lay {
     // the row's y index, x' = (x + y) mod m.  Pencils along x of different rows then start in different banks, and
     // every other access pattern still touches the same set of addresses per row.
     static __device__ __forceinline__ int rot(int j) {
+        constexpr int R = ROTM > 0 ? ROTM : 1;
         if (ROTM > 0) {
-            const int row = j / ROTM;
-            int x = j - row * ROTM + row % ROTM;
-            if (x >= ROTM) x -= ROTM;
-            return row * ROTM + x;
+            const int row = j / R;
+            int x = j - row * R + row % R;
+            if (x >= R) x -= R;
+            return row * R + x;
         }
         return j;
     }
@@ -966,6 +967,25 @@ __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(co
         if (bad) atomicOr(p.flag, 1);
     }
     __syncthreads();
+    // Stage-combine inputs u^n and u^(i-1) of this thread's rows: issued before the last projection sweep so that
+    // their latency is covered by it (same ownership as load_own_modes: modes g, g+G, ... of every variable).
+    constexpr int CG = NT / C;
+    constexpr int CNK = (Np + CG - 1) / CG;
+    double wn[CNK][V], wp[CNK][V];
+#define LOAD_COMBINE_INPUTS()                                                                               \
+    do {                                                                                                    \
+        const bool need_n = !p.rhs_only, need_p = !p.rhs_only && p.rk_b != 0.0;                             \
+        const double *bn = p.w_n + (size_t)((tid / C) * V) * p.ncells + cg;                                 \
+        const double *bp = p.w_prev + (size_t)((tid / C) * V) * p.ncells + cg;                              \
+        _Pragma("unroll") for (int k = 0; k < CNK; ++k) _Pragma("unroll") for (int v = 0; v < V; ++v) {     \
+            wn[k][v] = wp[k][v] = 0.0;                                                                      \
+            if (tid / C + k * CG < Np) {                                                                    \
+                if (need_n) wn[k][v] = __ldg(row_ptr(bn, k * CG * V + v, p.ncells));                        \
+                if (need_p) wp[k][v] = __ldg(row_ptr(bp, k * CG * V + v, p.ncells));                        \
+            }                                                                                               \
+        }                                                                                                   \
+    } while (0)
+
     // V4 + V5: weak-form derivative in nodal space, N = sum_a S_a G_a, then projection on the modes,
     //          dw += pref * (x)_a VtG N; alpha row: projection of the source only
     {
@@ -1011,6 +1031,7 @@ __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(co
                 }
             }
             __syncthreads();
+            LOAD_COMBINE_INPUTS();
             if (D == 3) {
                 sweep<DG_SEL_VTG, M, Np, M * M, C, NT, 1, true, true, L>(RX, 0, 0, ACC, 0, Vc, pref, tid);
                 if (AV) sweep<DG_SEL_VTG, M, Np, M * M, C, NT, 1, true, true, L>(RA, Vc, 0, ACC, Vc, 1, pref, tid);
@@ -1030,6 +1051,7 @@ __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(co
                 __syncthreads();
             }
             constexpr int SL = (D == 3) ? M * M : M;
+            LOAD_COMBINE_INPUTS();
             sweep<DG_SEL_VTG, M, Np, SL, C, NT, 1, true, true, L>(RX, 0, 0, ACC, 0, Vc, pref, tid);
             if (AV) sweep<DG_SEL_VTG, M, Np, SL, C, NT, 1, true, true, L>(RA, Vc, 0, ACC, Vc, 1, pref, tid);
             __syncthreads();
@@ -1042,27 +1064,14 @@ __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(co
     const double cdt = p.rhs_only ? 1.0 : p.rk_c * p.scal[0];
     double sA = 0.0, sB = 0.0, dA = 0.0, dB = 0.0;
     {
-        // same ownership as load_own_modes: modes g, g+G, ... of every variable of cell cl
-        constexpr int G = NT / C;
-        constexpr int NK = (Np + G - 1) / G;
+        constexpr int G = CG;
+        constexpr int NK = CNK;
         const int g = tid / C;
         const bool active = cell0 + cl < p.ncells;
-        const bool need_n = !p.rhs_only, need_p = !p.rhs_only && p.rk_b != 0.0;
-        const double *bn = p.w_n + (size_t)(g * V) * p.ncells + cg;
-        const double *bp = p.w_prev + (size_t)(g * V) * p.ncells + cg;
         double *bo = p.w_out + (size_t)(g * V) * p.ncells + cg;
 #pragma unroll
         for (int k = 0; k < NK; ++k) {
             const int mode = g + k * G;
-            double wn[V], wp[V];
-#pragma unroll
-            for (int v = 0; v < V; ++v) {
-                wn[v] = wp[v] = 0.0;
-                if (mode < Np) {
-                    if (need_n) wn[v] = __ldg(row_ptr(bn, k * G * V + v, p.ncells));
-                    if (need_p) wp[v] = __ldg(row_ptr(bp, k * G * V + v, p.ncells));
-                }
-            }
             int rem = mode, top = 0;
 #pragma unroll
             for (int a = 0; a < D; ++a) {
@@ -1074,11 +1083,11 @@ __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(co
                 if (mode < Np) {
                     const double Ld = ACC[L::at2(v, mode) * C + cl];
                     double wnew = Ld;
-                    if (!p.rhs_only) wnew = fma(cdt, Ld, fma(p.rk_b, wp[v], p.rk_a * wn[v]));
+                    if (!p.rhs_only) wnew = fma(cdt, Ld, fma(p.rk_b, wp[k][v], p.rk_a * wn[k][v]));
                     if (active) *row_ptr(bo, k * G * V + v, p.ncells) = wnew;
                     if (p.do_wavespeed) RA[L::at2(v, mode) * C + cl] = wnew;
                     if (AV && p.do_sensor && v == 0) {
-                        const double w = wn[v];
+                        const double w = wn[k][v];
                         sB = fma(w, w, sB);
                         dB = fma(w, Ld, dB);
                         if (top && M > 1) {
@@ -1090,6 +1099,7 @@ __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(co
             }
         }
     }
+#undef LOAD_COMBINE_INPUTS
     if (AV && p.do_sensor) {
         // lanes of a warp that share a cell (lane = cl + C*j), then one partial per warp and cell in `sens`
         constexpr int NW = NT / 32;

@@ -211,7 +211,7 @@ def ns_flux(u, grad, a: int, d: int, gamma: float, nu: float, chi: float):
 # ----------------------------------------------------------------------------------------------------
 def ssprk_tableau(stages: int):
     """PAPER.md:200: SSP Runge-Kutta, stages by order.  1: forward Euler; 2: SSP-RK2 (Heun);
-    3: SSP-RK3 (Shu-Osher; BASELINE config 1)."""
+    3: SSP-RK3 (Shu-Osher; BASELINE config 1); 5: SSPRK(5,4) for order >= 4."""
     if stages == 1:
         return [[1.0]], [[1.0]]
     if stages == 2:
@@ -219,7 +219,23 @@ def ssprk_tableau(stages: int):
     if stages == 3:
         return ([[1.0], [0.75, 0.25], [1.0 / 3.0, 0.0, 2.0 / 3.0]],
                 [[1.0], [0.0, 0.25], [0.0, 0.0, 2.0 / 3.0]])
-    raise ValueError("rk_stages must be 1, 2 or 3")
+    if stages == 5:
+        # 4th-order, five-stage SSP scheme in Shu-Osher form -- the scheme the paper selects for order >= 4
+        # ("fourth-order five stage" after Schaal et al. 2015, App. D, which is not in the
+        # container).  The coefficients are the optimal SSPRK(5,4) set of Spiteri & Ruuth (2002) as commonly
+        # published; reading A19b: "parity unpinned" against the authors' table, pinned as mathematics
+        # by the eight order-4 conditions, convexity (SSP) and the degree-4 Taylor polynomial on dw/dt = -w.
+        return ([[1.0],
+                 [0.444370493651235, 0.555629506348765],
+                 [0.620101851488403, 0.0, 0.379898148511597],
+                 [0.178079954393132, 0.0, 0.0, 0.821920045606868],
+                 [0.0, 0.0, 0.517231671970585, 0.096059710526147, 0.386708617503269]],
+                [[0.391752226571890],
+                 [0.0, 0.368410593050371],
+                 [0.0, 0.0, 0.251891774271694],
+                 [0.0, 0.0, 0.0, 0.544974750228521],
+                 [0.0, 0.0, 0.0, 0.063692468666290, 0.226007483236906]])
+    raise ValueError("rk_stages must be 1, 2, 3 or 5")
 
 
 @dataclass

@@ -393,6 +393,56 @@ def test_rk_tableaux_linear_ode():
         assert np.allclose(o.w, 1.7 * poly(0.3), rtol=1e-15)
 
 
+def test_ssprk54_order_conditions_and_convexity():
+    """five-stage fourth-order SSP-RK for order >= 4.  Pins of the tableau that do not depend on
+    the tableau's source: Shu-Osher rows are convex combinations (SSP property), the equivalent Butcher tableau
+    meets all eight order conditions up to order 4, and one step of dw/dt = -w is the degree-4 Taylor polynomial
+    plus a z^5 term with a coefficient other than 1/120 (the scheme is exactly fourth order, not fifth)."""
+    A, B = orc.ssprk_tableau(5)
+    s = 5
+    for i in range(s):
+        assert all(a >= 0.0 for a in A[i]) and all(b >= 0.0 for b in B[i])
+        assert abs(sum(A[i]) - 1.0) < 2e-15
+    K = np.zeros((s + 1, s))                      # u^(i) = u + dt sum_j K[i][j] L(u^(j))
+    for i in range(s):
+        for k in range(i + 1):
+            K[i + 1] += A[i][k] * K[k]
+            K[i + 1][k] += B[i][k]
+    a, b = K[:s], K[s]
+    c = a.sum(axis=1)
+    conds = [b.sum() - 1, b @ c - 1 / 2, b @ c ** 2 - 1 / 3, b @ a @ c - 1 / 6, b @ c ** 3 - 1 / 4,
+             b @ (c * (a @ c)) - 1 / 8, b @ a @ c ** 2 - 1 / 12, b @ a @ a @ c - 1 / 24]
+    assert np.max(np.abs(conds)) < 5e-15, conds
+
+    class Lin(orc.DGOracle):
+        def rhs(self, w, terms=False):
+            return -w
+    errs = []
+    for z in (0.4, 0.2):
+        o = Lin(2, (2, 2), 0.5, 2, 1.4, options=orc.Options(rk_stages=5, fixed_dt=z))
+        o.w[:] = 1.0
+        o.step(1)
+        taylor4 = 1 - z + z ** 2 / 2 - z ** 3 / 6 + z ** 4 / 24
+        errs.append(o.w.flat[0] - taylor4)
+    assert abs(errs[0]) < 0.4 ** 5 and abs(errs[1]) < 0.2 ** 5
+    assert abs(errs[0] / errs[1] - 32.0) < 1e-6          # the remainder is a pure z^5 term
+    assert abs(errs[1] / (-0.2 ** 5) - 1 / 120) > 1e-4   # ... whose coefficient is not exp's: order exactly 4
+
+
+def test_ssprk54_fourth_order_on_a_nonlinear_ode():
+    """dw/dt = -w^2, w(0) = 1 has w(t) = 1/(1+t): the global error at t = 1 drops by 2^4 per halving of dt."""
+    class Sq(orc.DGOracle):
+        def rhs(self, w, terms=False):
+            return -w * w
+    errs = []
+    for nst in (8, 16, 32):
+        o = Sq(2, (2, 2), 0.5, 2, 1.4, options=orc.Options(rk_stages=5, fixed_dt=1.0 / nst))
+        o.w[:] = 1.0
+        o.step(nst)
+        errs.append(abs(o.w.flat[0] - 0.5))
+    assert 14.0 < errs[0] / errs[1] < 18.0 and 14.0 < errs[1] / errs[2] < 18.0, errs
+
+
 def test_eq23_timestep_closed_form():
     """PAPER.md:204 (Eq. 23), p = n+1: uniform state => dt = f h / (2 (n+1) (c_s + |v|))."""
     for d, n in [(2, 1), (3, 3)]:

@@ -53,7 +53,8 @@ typedef struct dg_mesh {
 /* Runtime options; defaults are the paper's. */
 typedef struct dg_options {
     double f_cfl;        /* Courant factor of Eq. 23; default 0.5 */
-    int    rk_stages;    /* 1, 2 or 3: SSP-RK in Shu-Osher form; default 3 */
+    int    rk_stages;    /* 1, 2, 3: SSP-RK in Shu-Osher form, default 3; 5: the five-stage fourth-order
+                          * SSP scheme the paper uses for order >= 4 (two more state buffers) */
     int    av_enable;    /* 1: carry the artificial-viscosity field alpha; default 0 */
     double f_v;          /* shock source factor, Eq. 43; default 2.5 */
     double f_tau;        /* decay time factor, Eq. 44; default 0.5 */

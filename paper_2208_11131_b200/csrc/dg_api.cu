@@ -111,7 +111,7 @@ struct dg_solver {
     size_t nstate;          // V * M * ncells doubles
     Dispatch fn;
     cudaStream_t stream;
-    double *W0, *WA, *WB;
+    double *W0, *WA, *WB, *WC, *WD;   // u^n and stage buffers (WC, WD: five-stage scheme only)
     double *flux;           // dim * Vc * m^(dim-1) * ncells doubles: projected upper-face fluxes of the current stage
     double *scal;           // [0] dt, [1] t, [2] cmax, [3] vmax, [8..12] totals
     unsigned long long *maxbits;
@@ -139,6 +139,8 @@ size_t workspace_layout(dg_solver *s, char *base) {
     s->W0 = (double *)take(sb);
     s->WA = (double *)take(sb);
     s->WB = (s->opt.rk_stages >= 3) ? (double *)take(sb) : nullptr;
+    s->WC = (s->opt.rk_stages == 5) ? (double *)take(sb) : nullptr;
+    s->WD = (s->opt.rk_stages == 5) ? (double *)take(sb) : nullptr;
     s->flux = (double *)take((size_t)s->dim * s->Vc * (s->M / s->order) * s->ncells * sizeof(double));
     s->scal = (double *)take(16 * sizeof(double));
     s->maxbits = (unsigned long long *)take(2 * sizeof(unsigned long long));
@@ -166,7 +168,8 @@ int validate(const dg_mesh *mesh, int order, double gamma, double nu, double chi
     if (!(mesh->h > 0.0) || !std::isfinite(mesh->h)) return fail(DG_EINVAL, "mesh.h must be positive");
     if (!(gamma > 1.0)) return fail(DG_EINVAL, "gamma must exceed 1");
     if (!(nu >= 0.0) || !(chi >= 0.0)) return fail(DG_EINVAL, "nu and chi must be non-negative");
-    if (o->rk_stages < 1 || o->rk_stages > 3) return fail(DG_EINVAL, "rk_stages must be 1, 2 or 3");
+    if (o->rk_stages != 1 && o->rk_stages != 2 && o->rk_stages != 3 && o->rk_stages != 5)
+        return fail(DG_EINVAL, "rk_stages must be 1, 2, 3 or 5");
     if (!(o->f_cfl > 0.0) && !(o->fixed_dt > 0.0)) return fail(DG_EINVAL, "f_cfl must be positive");
     return DG_OK;
 }
@@ -208,12 +211,45 @@ int enqueue_wavespeed(dg_solver *s) {
 
 // enqueue one full SSP-RK step (Shu-Osher forms)
 int enqueue_step(dg_solver *s) {
-    static const double A0[3][3] = {{1.0, 0, 0}, {1.0, 0.5, 0}, {1.0, 0.75, 1.0 / 3.0}};
-    static const double B1[3][3] = {{0.0, 0, 0}, {0.0, 0.5, 0}, {0.0, 0.25, 2.0 / 3.0}};
-    static const double CC[3][3] = {{1.0, 0, 0}, {1.0, 0.5, 0}, {1.0, 0.25, 2.0 / 3.0}};
     const int S = s->opt.rk_stages;
     dg_dt_kernel<<<1, 1, 0, s->stream>>>(s->scal, s->maxbits, s->opt.f_cfl, s->h, s->order, s->opt.fixed_dt);
     CU(cudaGetLastError());
+    if (S == 5) {
+        // SSPRK(5,4) (coefficients: DESIGN.md reading A19b).  Stages 1-4 have the three-term form
+        // u^(i) = a u^n + b u^(i-1) + c dt L(u^(i-1)); stage 4 also writes AUX = a' u^(2) + b' u^(3) + c' dt L(u^(3)),
+        // so that the last stage is again three terms: u^(n+1) = AUX + b u^(4) + c dt L(u^(4)).
+        static const double a[5] = {1.0, 0.444370493651235, 0.620101851488403, 0.178079954393132, 1.0};
+        static const double b[5] = {0.0, 0.555629506348765, 0.379898148511597, 0.821920045606868, 0.386708617503269};
+        static const double c[5] = {0.391752226571890, 0.368410593050371, 0.251891774271694, 0.544974750228521,
+                                    0.226007483236906};
+        const double *prev[5] = {s->W0, s->WA, s->WB, s->WC, s->WA};
+        double *out[5] = {s->WA, s->WB, s->WC, s->WA, s->W0};
+        for (int i = 0; i < 5; ++i) {
+            DgStageArgs g;
+            fill_args(s, &g);
+            g.w_prev = prev[i];
+            g.w_n = (i == 4) ? s->WD : s->W0;
+            g.w_out = out[i];
+            g.rk_a = a[i];
+            g.rk_b = b[i];
+            g.rk_c = c[i];
+            if (i == 3) {
+                g.w_aux_in = s->WB;
+                g.w_aux = s->WD;
+                g.aux_a = 0.517231671970585;
+                g.aux_b = 0.096059710526147;
+                g.aux_c = 0.063692468666290;
+            }
+            g.do_sensor = (i == 0) && s->av;
+            g.commit_sensor = (i == 4) && s->av;
+            g.do_wavespeed = (i == 4);
+            CU(s->fn.launch(s->visc, s->av, &g, s->stream, 0));
+        }
+        return DG_OK;
+    }
+    static const double A0[3][3] = {{1.0, 0, 0}, {1.0, 0.5, 0}, {1.0, 0.75, 1.0 / 3.0}};
+    static const double B1[3][3] = {{0.0, 0, 0}, {0.0, 0.5, 0}, {0.0, 0.25, 2.0 / 3.0}};
+    static const double CC[3][3] = {{1.0, 0, 0}, {1.0, 0.5, 0}, {1.0, 0.25, 2.0 / 3.0}};
     double *buf[2] = {s->WA, s->WB};
     const double *prev = s->W0;
     for (int i = 0; i < S; ++i) {

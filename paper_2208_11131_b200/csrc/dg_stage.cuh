@@ -1085,6 +1085,11 @@ __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(co
                     double wnew = Ld;
                     if (!p.rhs_only) wnew = fma(cdt, Ld, fma(p.rk_b, wp[k][v], p.rk_a * wn[k][v]));
                     if (active) *row_ptr(bo, k * G * V + v, p.ncells) = wnew;
+                    if (p.w_aux != nullptr && active) {
+                        // SSPRK(5,4): the part of the last stage that is known now (u^(2), u^(3), L(u^(3)))
+                        const size_t gi = (size_t)((g + k * G) * V + v) * p.ncells + cg;
+                        p.w_aux[gi] = fma(p.aux_c * p.scal[0], Ld, fma(p.aux_b, wp[k][v], p.aux_a * p.w_aux_in[gi]));
+                    }
                     if (p.do_wavespeed) RA[L::at2(v, mode) * C + cl] = wnew;
                     if (AV && p.do_sensor && v == 0) {
                         const double w = wn[k][v];

@@ -5,6 +5,8 @@ struct DgStageArgs {
     const double *w_prev;   // stage input u^(i-1): halo + own reads
     const double *w_n;      // u^n (own cell only)
     double *w_out;          // u^(i) (may alias w_n on the last stage); or dw/dt if rhs_only
+    const double *w_aux_in; // SSPRK(5,4) stage 4 only: u^(2); NULL otherwise
+    double *w_aux;          // SSPRK(5,4) stage 4 only: aux_a u^(2) + aux_b u^(i-1) + aux_c dt L(u^(i-1)); NULL otherwise
     double *flux;           // projected upper-face fluxes [axis][var][transverse mode][cell] (face kernel -> stage kernel)
     const double *scal;     // device scalars: [0] = dt
     unsigned long long *maxbits;  // [0] = bits of max c_s, [1] = bits of max |v| (non-negative doubles)
@@ -15,5 +17,6 @@ struct DgStageArgs {
     double h, gamma, nu, chi;
     double f_v, f_tau, f_w, s_onset, alpha_max;
     double rk_a, rk_b, rk_c;  // u^(i) = rk_a u^n + rk_b u^(i-1) + rk_c dt L(u^(i-1))
+    double aux_a, aux_b, aux_c;
     int do_sensor, do_wavespeed, commit_sensor, rhs_only;
 };

@@ -143,6 +143,31 @@ def test_lower_rk_parity(stages):
     assert np.all(parity_norm(g.get_state(), o.get_state(), wl) <= 1e-11)
 
 
+@pytest.mark.parametrize("cfg", [4, 2])
+def test_ssprk54_parity(cfg):
+    """Five-stage fourth-order SSP-RK against the oracle's Shu-Osher loop."""
+    wl = _scaled_config(cfg)
+    w0 = wk.initial_modes(wl)
+    o = make_oracle(wl, rk_stages=5)
+    g = make_gpu(wl, rk_stages=5)
+    o.set_state(w0)
+    g.set_state(w0)
+    assert o.step(1) == 0
+    g.step(1)
+    e1 = parity_norm(g.get_state(), o.get_state(), wl)
+    assert np.all(e1 <= TOL_1), e1
+    assert o.step(4) == 0
+    g.step(4)
+    e5 = parity_norm(g.get_state(), o.get_state(), wl)
+    assert np.all(e5 <= TOL_10), e5
+    if wl.av:
+        assert np.max(np.abs(g.get_alpha() - o.get_alpha())) <= TOL_10
+    tg, dtg = g.get_time()
+    assert abs(tg - o.t) <= 1e-14 * o.t
+    _report("%s SSPRK(5,4) mesh %s: 1 step %.3e, 5 steps %.3e" % (wl.name, "x".join(map(str, wl.ncell)),
+                                                                 np.max(e1), np.max(e5)))
+
+
 def test_fixed_dt_and_time():
     wl = _scaled_config(1)
     w0 = wk.initial_modes(wl)

@@ -19,6 +19,7 @@ Legendre values by three-term recurrence, every step in the paper's order and no
   O10 sensor           PAPER.md:347-365 (Eq. 41-42), 392-397 (Eq. 45); top set / lagging per A13/A15
   O11 SSP-RK           PAPER.md:200 (Shu-Osher forms; 3-stage default per BASELINE config 1)
   O12 totals           PAPER.md:127, 423 (mode 0 is the cell mean)
+  O13 positivity lim.  PAPER.md:417-432 (Eq. 47), optional, after every RK stage (readings L1-L6 in DESIGN.md)
 
 Parity pins (tests/test_oracle_*.py) cover every function here; the readings with no pin in the paper
 (A6, A11, A12, A14, A15, A18 in DESIGN.md) are "parity unpinned" against the authors' code but pinned as
@@ -250,6 +251,7 @@ class Options:
     s_onset0: float = 1.0e-4
     alpha_max: float = 1.0
     fixed_dt: float = 0.0  # > 0: use this dt instead of Eq. 23
+    limiter_enable: bool = False  # positivity limiter after every RK stage (Eq. 47)
 
 
 class DGOracle:
@@ -482,6 +484,44 @@ class DGOracle:
         return S, G
 
     # ---- O11: one SSP-RK step -----------------------------------------------------------------------
+    # ---- O13: positivity limiter (Eq. 47) ---------------------------------------------
+    def positivity_limit(self, w):
+        """Returns the limited copy of w[cell, mode, var].  Per cell, in the paper's order:
+        mean density rho_bar = w_0 and mean pressure p_bar (pressure of the cell-mean state, reading L2); either
+        <= 0: "a code crash is unavoidable" -> unphysical flag, cell left alone.  Evaluation points = union of the
+        volume Gauss points and the Gauss points of the 2d faces (PAPER.md:427).  Density: rho_bottom = 1e-6 rho_bar;
+        if rho_min < rho_bottom, f = (rho_bar - rho_bottom)/(rho_bar - rho_min) and every mode but the mean of every
+        conserved field is multiplied by f (Eq. 47; "l > 1" counts modes from 1, reading L1).  Pressure: p_bottom =
+        1e-6 p_bar (reading L3); while p_min < p_bottom multiply the same modes by 0.5.  The
+        artificial-viscosity field alpha is not a hydrodynamic field and is left untouched (reading L5)."""
+        Vc = self.Vc
+        w = w.copy()
+        if self.M == 1:
+            return w                                        # no higher modes to limit
+        E = np.concatenate([self.Phi] + [self.PhiF[a][s] for a in range(self.d) for s in (0, 1)], axis=0)
+        for c in range(self.ncells):
+            mean = w[c, 0, :Vc].copy()
+            rho_bar = mean[0]
+            p_bar = (self.gamma - 1.0) * (mean[1 + self.d] - 0.5 * float(np.sum(mean[1:1 + self.d] ** 2)) / rho_bar) \
+                if rho_bar > 0.0 else -1.0
+            if not (rho_bar > 0.0) or not (p_bar > 0.0):
+                self.unphysical = True
+                continue
+            u = E @ w[c, :, :Vc]                            # [point, var]
+            rho_bottom = 1.0e-6 * rho_bar
+            rho_min = float(np.min(u[:, 0]))
+            if rho_min < rho_bottom:
+                f = (rho_bar - rho_bottom) / (rho_bar - rho_min)
+                w[c, 1:, :Vc] *= f
+            p_bottom = 1.0e-6 * p_bar
+            for _ in range(64):
+                u = E @ w[c, :, :Vc]
+                pr = (self.gamma - 1.0) * (u[:, 1 + self.d] - 0.5 * np.sum(u[:, 1:1 + self.d] ** 2, axis=1) / u[:, 0])
+                if float(np.min(pr)) >= p_bottom:
+                    break
+                w[c, 1:, :Vc] *= 0.5
+        return w
+
     def step(self, nsteps=1):
         A, B = ssprk_tableau(self.opt.rk_stages)
         for _ in range(nsteps):
@@ -499,6 +539,8 @@ class DGOracle:
                         unew += A[i][k] * us[k]
                     if B[i][k] != 0.0:
                         unew += (B[i][k] * dt) * Ls[k]
+                if self.opt.limiter_enable:
+                    unew = self.positivity_limit(unew)
                 us.append(unew)
             self.w = us[-1]
             if self.av:

@@ -63,6 +63,7 @@ typedef struct dg_options {
     double alpha_max;    /* clamp of the point-wise alpha used in Eq. 46; default 1 */
     double fixed_dt;     /* > 0: use this dt instead of Eq. 23; default 0 */
     int    use_graph;    /* 1: replay each time step as a CUDA graph (default); 0: plain launches */
+    int    limiter_enable; /* 1: positivity limiter (Eq. 47) on the output of every RK stage; default 0 */
 } dg_options;
 
 /* Fill *opt with the defaults above. */
@@ -116,6 +117,11 @@ int dg_conserved_totals(dg_solver *s, double totals[5]);
 /* Evaluate dw/dt = L(w) (Eq. 20) of the current state without advancing it, for term-wise parity tests:
  * out has the layout of the state (count = Vc*M*Ncells); alpha_out (may be NULL) that of alpha. */
 int dg_eval_rhs(dg_solver *s, double *out, size_t count, double *alpha_out, size_t alpha_count);
+
+/* Apply the positivity limiter (Eq. 47) once to the current state, whatever `limiter_enable` says
+ * (term-level parity tests; dg_step applies it after every RK stage when the option is on).  Returns
+ * DG_EUNPHYSICAL if a cell mean has rho <= 0 or p <= 0. */
+int dg_apply_limiter(dg_solver *s);
 
 /* Simulation time and the last timestep used (host pointers, either may be NULL). */
 int dg_get_time(dg_solver *s, double *t, double *last_dt);

@@ -32,15 +32,18 @@ typedef cudaError_t (*launch_fn)(int, int, const DgStageArgs *, cudaStream_t, in
 typedef cudaError_t (*upload_fn)(const DgTables *);
 typedef void (*info_fn)(int, int, int *, int *, int *);
 typedef cudaError_t (*config_fn)(int, int);
+typedef cudaError_t (*limit_fn)(double *, int, int, double, int *, cudaStream_t);
 
 struct Dispatch {
     launch_fn launch;
     upload_fn upload;
     info_fn info;
     config_fn config;
+    limit_fn limit;
 };
 
-#define DG_ENTRY(d, m) {DG_FN(dg_launch, d, m), DG_FN(dg_upload, d, m), DG_FN(dg_info, d, m), DG_FN(dg_config, d, m)},
+#define DG_ENTRY(d, m) {DG_FN(dg_launch, d, m), DG_FN(dg_upload, d, m), DG_FN(dg_info, d, m), DG_FN(dg_config, d, m), \
+                        DG_FN(dg_limit, d, m)},
 const Dispatch kDispatch[2][8] = {{DG_FOR_ALL_M(DG_ENTRY, 2)}, {DG_FOR_ALL_M(DG_ENTRY, 3)}};
 
 // ---- helper kernels -------------------------------------------------------------------------------
@@ -209,8 +212,26 @@ int enqueue_wavespeed(dg_solver *s) {
     return DG_OK;
 }
 
+// positivity limiter on a stage output (optional).  Nothing to limit for degree 0.
+int enqueue_limiter(dg_solver *s, double *w) {
+    if (!s->opt.limiter_enable || s->order < 2) return DG_OK;
+    CU(s->fn.limit(w, s->V, s->ncells, s->gamma, s->flag, s->stream));
+    return DG_OK;
+}
+
+// with the limiter on, the wave speeds of the new state (Eq. 23) are taken after it, by the stand-alone kernel
+int enqueue_post_step(dg_solver *s) {
+    if (!s->opt.limiter_enable || s->order < 2) return DG_OK;
+    DgStageArgs a;
+    fill_args(s, &a);
+    a.w_prev = s->W0;
+    CU(s->fn.launch(s->visc, s->av, &a, s->stream, 1));
+    return DG_OK;
+}
+
 // enqueue one full SSP-RK step (Shu-Osher forms)
 int enqueue_step(dg_solver *s) {
+    const bool lim = s->opt.limiter_enable && s->order >= 2;
     const int S = s->opt.rk_stages;
     dg_dt_kernel<<<1, 1, 0, s->stream>>>(s->scal, s->maxbits, s->opt.f_cfl, s->h, s->order, s->opt.fixed_dt);
     CU(cudaGetLastError());
@@ -242,10 +263,12 @@ int enqueue_step(dg_solver *s) {
             }
             g.do_sensor = (i == 0) && s->av;
             g.commit_sensor = (i == 4) && s->av;
-            g.do_wavespeed = (i == 4);
+            g.do_wavespeed = (i == 4) && !lim;
             CU(s->fn.launch(s->visc, s->av, &g, s->stream, 0));
+            int rc = enqueue_limiter(s, out[i]);
+            if (rc) return rc;
         }
-        return DG_OK;
+        return enqueue_post_step(s);
     }
     static const double A0[3][3] = {{1.0, 0, 0}, {1.0, 0.5, 0}, {1.0, 0.75, 1.0 / 3.0}};
     static const double B1[3][3] = {{0.0, 0, 0}, {0.0, 0.5, 0}, {0.0, 0.25, 2.0 / 3.0}};
@@ -264,12 +287,14 @@ int enqueue_step(dg_solver *s) {
         a.rk_c = CC[S - 1][i];
         a.do_sensor = (i == 0) && s->av;
         a.commit_sensor = (i == S - 1) && s->av;
-        a.do_wavespeed = (i == S - 1);
+        a.do_wavespeed = (i == S - 1) && !lim;
         CU(s->fn.launch(s->visc, s->av, &a, s->stream, 0));
+        int rc = enqueue_limiter(s, out);
+        if (rc) return rc;
         prev = out;
     }
     if (S == 1) CU(cudaMemcpyAsync(s->W0, s->WA, s->nstate * sizeof(double), cudaMemcpyDeviceToDevice, s->stream));
-    return DG_OK;
+    return enqueue_post_step(s);
 }
 
 int check_flag(dg_solver *s) {
@@ -384,6 +409,7 @@ int dg_default_options(dg_options *opt) {
     opt->alpha_max = 1.0;
     opt->fixed_dt = 0.0;
     opt->use_graph = 1;
+    opt->limiter_enable = 0;
     return DG_OK;
 }
 
@@ -449,7 +475,9 @@ int dg_step_async(dg_solver *s, int nsteps) {
         int rc = enqueue_wavespeed(s);
         if (rc) return rc;
     }
-    const int per_step = 1 + 2 * s->opt.rk_stages;   // dt kernel + (face, stage) per RK stage
+    const bool lim = s->opt.limiter_enable && s->order >= 2;
+    // dt kernel + (face, stage[, limiter]) per RK stage [+ wave-speed kernel]
+    const int per_step = 1 + (2 + (lim ? 1 : 0)) * s->opt.rk_stages + (lim ? 1 : 0);
     if (s->opt.use_graph && nsteps > 0) {
         if (!s->graph) {
             cudaStream_t cap = s->stream;
@@ -600,6 +628,18 @@ int dg_profile_stage(dg_solver *s, int reps, double *face_ms, double *stage_ms) 
     if (rc) return rc;
     if (face_ms) *face_ms = tf / reps;
     if (stage_ms) *stage_ms = ts / reps;
+    return check_flag(s);
+}
+
+int dg_apply_limiter(dg_solver *s) {
+    if (!s) return fail(DG_EINVAL, "solver is NULL");
+    // a state that needs limiting has already been flagged by the wave-speed pass of dg_set_state: start afresh
+    CU(cudaMemsetAsync(s->flag, 0, sizeof(int), s->stream));
+    if (s->order >= 2) {
+        CU(s->fn.limit(s->W0, s->V, s->ncells, s->gamma, s->flag, s->stream));
+        s->launches += 1;
+        s->speeds_valid = false;
+    }
     return check_flag(s);
 }
 

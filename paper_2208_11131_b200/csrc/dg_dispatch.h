@@ -14,7 +14,8 @@ struct DgTables;
                                        int wavespeed_only);                                            \
     cudaError_t DG_FN(dg_upload, d, m)(const DgTables *t);                                             \
     void DG_FN(dg_info, d, m)(int visc, int av, int *c, int *nt, int *smem);                           \
-    cudaError_t DG_FN(dg_config, d, m)(int visc, int av);
+    cudaError_t DG_FN(dg_config, d, m)(int visc, int av);                                              \
+    cudaError_t DG_FN(dg_limit, d, m)(double *w, int V, int ncells, double gamma, int *flag, cudaStream_t st);
 
 #define DG_FOR_ALL_M(X, d) X(d, 1) X(d, 2) X(d, 3) X(d, 4) X(d, 5) X(d, 6) X(d, 7) X(d, 8)
 

@@ -2,6 +2,7 @@
 // (Euler, NS, AV, NS+AV) and exports plain launch functions for dg_api.cu.  Compiled 16 times by build.py
 // with -DDG_DIM=2|3 -DDG_M=1..8 (keeps ptxas work parallel and each image small).
 #include "dg_stage.cuh"
+#include "dg_limiter.cuh"
 #include "dg_dispatch.h"
 
 #ifndef DG_DIM
@@ -19,6 +20,9 @@ cudaError_t configure() {
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(dgk::dg_face_kernel<DG_DIM, DG_M, VISC, AV>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              dgk::FaceCfg<DG_DIM, DG_M, VISC, AV>::kSmemBytes);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(dgk::dg_limiter_kernel<DG_DIM, DG_M>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             dgk::LimCfg<DG_DIM, DG_M>::kSmemBytes);
     if (e != cudaSuccess) return e;
     return cudaFuncSetAttribute(dgk::dg_wavespeed_kernel<DG_DIM, DG_M, VISC, AV>,
                                 cudaFuncAttributeMaxDynamicSharedMemorySize, K::kSmemBytes);
@@ -60,6 +64,14 @@ cudaError_t DG_FN(dg_launch, DG_DIM, DG_M)(int visc, int av, const DgStageArgs *
     if (visc) return launch<true, false>(*a, st, wavespeed_only);
     if (av) return launch<false, true>(*a, st, wavespeed_only);
     return launch<false, false>(*a, st, wavespeed_only);
+}
+
+// positivity limiter on a state buffer with V variables per mode (only the d+2 conserved ones are touched)
+cudaError_t DG_FN(dg_limit, DG_DIM, DG_M)(double *w, int V, int ncells, double gamma, int *flag, cudaStream_t st) {
+    using LK = dgk::LimCfg<DG_DIM, DG_M>;
+    const int blocks = (ncells + LK::C - 1) / LK::C;
+    dgk::dg_limiter_kernel<DG_DIM, DG_M><<<blocks, LK::NT, LK::kSmemBytes, st>>>(w, V, ncells, gamma, flag);
+    return cudaGetLastError();
 }
 
 cudaError_t DG_FN(dg_upload, DG_DIM, DG_M)(const DgTables *t) {

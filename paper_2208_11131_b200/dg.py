@@ -33,7 +33,7 @@ class dg_mesh(C.Structure):
 class dg_options(C.Structure):
     _fields_ = [("f_cfl", C.c_double), ("rk_stages", C.c_int), ("av_enable", C.c_int), ("f_v", C.c_double),
                 ("f_tau", C.c_double), ("f_w", C.c_double), ("s_onset0", C.c_double), ("alpha_max", C.c_double),
-                ("fixed_dt", C.c_double), ("use_graph", C.c_int)]
+                ("fixed_dt", C.c_double), ("use_graph", C.c_int), ("limiter_enable", C.c_int)]
 
 
 # every symbol include/dg.h declares: name -> (restype, argtypes)
@@ -58,6 +58,7 @@ SYMBOLS = {
     "dg_get_time": (C.c_int, [_P, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
     "dg_kernel_info": (C.c_int, [_P, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int)]),
     "dg_profile_stage": (C.c_int, [_P, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
+    "dg_apply_limiter": (C.c_int, [_P]),
     "dg_launch_count": (C.c_int, [_P, C.POINTER(C.c_longlong)]),
     "dg_measure_fp64_peak": (C.c_int, [C.c_int, C.POINTER(C.c_double), _P]),
     "dg_free": (C.c_int, [_P]),
@@ -217,6 +218,9 @@ class Solver:
         f, g = C.c_double(), C.c_double()
         _check(self._lib.dg_profile_stage(self._h, reps, C.byref(f), C.byref(g)))
         return f.value, g.value
+
+    def apply_limiter(self):
+        _check(self._lib.dg_apply_limiter(self._h))
 
     def launch_count(self):
         n = C.c_longlong()

@@ -312,3 +312,86 @@ def test_full_size_sampled_rhs_parity():
     mag = L_dev[0].abs().sum(dim=1).cpu().numpy()
     assert np.all(np.abs(tot) <= 1e-12 * mag), (tot, mag)
     _report("full-size cfg4 128^3 sampled dw/dt: worst relative difference %.3e over %d cells" % (worst, len(samples)))
+
+
+# ---------------------------------------------------------------------------------------------------
+# positivity limiter (Eq. 47)
+# ---------------------------------------------------------------------------------------------------
+def _rough_state(wl, seed):
+    """Smooth random state with a few violent cells: density and energy oscillations that push rho or p below zero
+    at volume or face points (decisions far from the thresholds, so both sides take the same ones)."""
+    Vc, M = wl.dim + 2, wl.modes
+    w0, al = wk.random_smooth_modes(wl.dim, wl.ncell, wl.degree, wl.gamma, seed=seed, amp=0.02,
+                                    nvar_extra=1 if wl.av else 0)
+    w = w0.reshape(M, Vc, -1)
+    rng = np.random.default_rng(seed + 100)
+    n = w.shape[2]
+    for c in rng.choice(n, size=max(3, n // 4), replace=False):
+        kind = rng.integers(3)
+        mode = 1 + int(rng.integers(M - 1))
+        if kind in (0, 2):
+            w[mode, 0, c] += rng.choice([-1.0, 1.0]) * (1.1 + rng.random())      # density
+        if kind in (1, 2):
+            w[mode, Vc - 1, c] += rng.choice([-1.0, 1.0]) * (2.5 + rng.random())  # energy -> pressure
+    return np.ascontiguousarray(w).ravel(), al
+
+
+LIM_CASES = [(2, (5, 3), 1, "euler"), (2, (5, 3), 3, "ns_av"), (3, (3, 2, 2), 2, "ns_av"), (3, (9, 4, 3), 3, "euler"),
+             (2, (37, 3), 4, "av"), (3, (2, 2, 2), 5, "euler"), (3, (2, 2, 3), 7, "euler")]
+
+
+@pytest.mark.parametrize("d,ncell,n,phys", LIM_CASES)
+def test_limiter_parity(d, ncell, n, phys):
+    wl = _wl(d, ncell, n, phys)
+    w0, al = _rough_state(wl, seed=21 + n)
+    o = make_oracle(wl)
+    g = make_gpu(wl)
+    o.set_state(w0)
+    g.set_state(w0)
+    if wl.av:
+        o.set_alpha(al)
+        g.set_alpha(al)
+    before = o.get_state().copy()
+    o.w = o.positivity_limit(o.w)
+    assert not o.unphysical
+    g.apply_limiter()
+    wo, wg = o.get_state(), g.get_state()
+    changed = np.any((wo != before).reshape(wl.modes, wl.dim + 2, -1), axis=(0, 1))
+    assert 0 < changed.sum() < changed.size                      # the limiter acted on some cells, not on all
+    scale = np.max(np.abs(before))
+    assert np.max(np.abs(wg - wo)) <= 1e-13 * scale
+    untouched = np.broadcast_to(~changed, (wl.modes, wl.dim + 2, changed.size)).ravel()
+    assert np.array_equal(wg[untouched], before[untouched])      # cells the oracle leaves alone are bit-identical
+    if wl.av:
+        assert np.array_equal(g.get_alpha(), al)
+    _report("limiter %dD degree %d mesh %s: %d of %d cells limited, max difference %.3e" % (
+        d, n, "x".join(map(str, ncell)), changed.sum(), changed.size, np.max(np.abs(wg - wo)) / scale))
+
+
+def test_limiter_steps_parity_and_inactive_bitwise():
+    # (a) smooth flow: the limiter never acts, results with and without it are bit-identical (PAPER.md:433)
+    wl = _scaled_config(4)
+    w0 = wk.initial_modes(wl)
+    res = []
+    for lim in (0, 1):
+        g = make_gpu(wl, limiter_enable=lim)
+        g.set_state(w0)
+        g.step(3)
+        res.append((g.get_state(), g.get_alpha(), g.get_time()))
+    assert np.array_equal(res[0][0], res[1][0]) and np.array_equal(res[0][1], res[1][1]) and res[0][2] == res[1][2]
+    # (b) rough start: limiter active inside the RK stages, oracle and GPU stay together
+    wl = _wl(2, (8, 4), 2, "av", f_cfl=0.1)
+    w0, al = _rough_state(wl, seed=7)
+    o = make_oracle(wl, limiter_enable=True)
+    g = make_gpu(wl, limiter_enable=1)
+    o.set_state(w0)
+    g.set_state(w0)
+    o.w = o.positivity_limit(o.w)                                 # start from an admissible state on both sides
+    g.apply_limiter()
+    assert o.step(2) == 0
+    g.step(2)
+    e = parity_norm(g.get_state(), o.get_state(), wl)
+    assert np.all(e <= 1e-10), e
+    tg, dtg = g.get_time()
+    assert abs(dtg - o.last_dt) <= 1e-12 * o.last_dt
+    _report("limiter inside RK3, 2D degree 2 AV, 2 steps from a limited rough state: %.3e" % np.max(e))

@@ -30,7 +30,7 @@ from paper_2208_11131_b200 import workloads as wk         # noqa: E402
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE dg_stage_kernel launch from the committed `ncu --set full`
 # capture (profiles/), keyed by (workload, degree); None where no capture exists.
-TRAFFIC_BYTES = {("cfg4", 3): 18.276837e9 + 6.423285e9}   # profiles/r1f_cfg4_two_kernel.md
+TRAFFIC_BYTES = {("cfg4", 3): 18.275670e9 + 6.422608e9}   # profiles/r1g_cfg4_final.md
 
 METRIC = "DG DoF-updates/sec (fp64, per RK stage)"
 UNIT = "DoF-updates/s"

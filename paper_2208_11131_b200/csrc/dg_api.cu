@@ -174,6 +174,12 @@ int validate(const dg_mesh *mesh, int order, double gamma, double nu, double chi
     if (o->rk_stages != 1 && o->rk_stages != 2 && o->rk_stages != 3 && o->rk_stages != 5)
         return fail(DG_EINVAL, "rk_stages must be 1, 2, 3 or 5");
     if (!(o->f_cfl > 0.0) && !(o->fixed_dt > 0.0)) return fail(DG_EINVAL, "f_cfl must be positive");
+    if (o->av_enable) {
+        if (!(o->f_tau > 0.0)) return fail(DG_EINVAL, "f_tau must be positive (Eq. 44 divides by it)");
+        if (!(o->f_v >= 0.0) || !(o->f_w >= 0.0)) return fail(DG_EINVAL, "f_v and f_w must be non-negative");
+        if (!(o->alpha_max >= 0.0)) return fail(DG_EINVAL, "alpha_max must be non-negative");
+        if (!(o->s_onset0 >= 0.0)) return fail(DG_EINVAL, "s_onset0 must be non-negative");
+    }
     return DG_OK;
 }
 
@@ -301,7 +307,12 @@ int check_flag(dg_solver *s) {
     int f = 0;
     CU(cudaMemcpyAsync(&f, s->flag, sizeof(int), cudaMemcpyDeviceToHost, s->stream));
     CU(cudaStreamSynchronize(s->stream));
-    if (f) return fail(DG_EUNPHYSICAL, "rho <= 0 or p <= 0 at an evaluation point%s");
+    if (f) {
+        char where[64];
+        std::snprintf(where, sizeof(where), " (%s%s%s%s)", (f & 1) ? "volume point " : "", (f & 2) ? "face point " : "",
+                      (f & 4) ? "wave-speed pass " : "", (f & 8) ? "limiter cell mean" : "");
+        return fail(DG_EUNPHYSICAL, "rho <= 0 or p <= 0 at an evaluation point%s", where);
+    }
     return DG_OK;
 }
 
@@ -375,6 +386,9 @@ int init_common(dg_solver **out, const dg_mesh *mesh, int order, double gamma, d
         e = s->fn.upload(&t);
     }
     if (e == cudaSuccess) e = cudaMemset(base, 0, need);
+    // the memset runs on the legacy stream and is asynchronous to the host: finish it before any later work on a
+    // caller-chosen (possibly non-blocking) stream can touch the workspace
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
     if (e != cudaSuccess) {
         if (s->owned) cudaFree(s->owned);
         delete s;
@@ -382,6 +396,21 @@ int init_common(dg_solver **out, const dg_mesh *mesh, int order, double gamma, d
     }
     s->fn.info(s->visc, s->av, &s->kC, &s->kNT, &s->kSmem);
     *out = s;
+    return DG_OK;
+}
+
+// zero `count` doubles behind a caller pointer that may be HOST or DEVICE memory (include/dg.h conventions)
+int zero_fill(dg_solver *s, double *dst, size_t count) {
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, dst) == cudaSuccess &&
+        (at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged)) {
+        CU(cudaMemsetAsync(dst, 0, count * sizeof(double), s->stream));
+        CU(cudaStreamSynchronize(s->stream));
+    } else {
+        cudaGetLastError();
+        CU(cudaStreamSynchronize(s->stream));
+        std::memset(dst, 0, count * sizeof(double));
+    }
     return DG_OK;
 }
 
@@ -497,8 +526,12 @@ int dg_step_async(dg_solver *s, int nsteps) {
             }
             s->stream = keep;
             if (tmp) cudaStreamDestroy(tmp);
-            if (rc) return rc;
-            if (e != cudaSuccess) return fail(DG_ECUDA, "graph capture failed: %s", cudaGetErrorString(e));
+            if (rc || e != cudaSuccess) {
+                if (g) cudaGraphDestroy(g);
+                cudaGetLastError();
+                if (rc) return rc;
+                return fail(DG_ECUDA, "graph capture failed: %s", cudaGetErrorString(e));
+            }
             e = cudaGraphInstantiate(&s->graph, g, 0);
             cudaGraphDestroy(g);
             if (e != cudaSuccess) return fail(DG_ECUDA, "cudaGraphInstantiate: %s", cudaGetErrorString(e));
@@ -537,17 +570,7 @@ int dg_get_state(dg_solver *s, double *w, size_t count) {
 int dg_get_alpha(dg_solver *s, double *alpha, size_t count) {
     if (!s || !alpha) return fail(DG_EINVAL, "NULL argument");
     if (count != (size_t)s->M * s->ncells) return fail(DG_EINVAL, "count must be M*Ncells");
-    if (!s->av) {
-        cudaPointerAttributes at;
-        if (cudaPointerGetAttributes(&at, alpha) == cudaSuccess && at.type == cudaMemoryTypeDevice) {
-            CU(cudaMemsetAsync(alpha, 0, count * sizeof(double), s->stream));
-            CU(cudaStreamSynchronize(s->stream));
-        } else {
-            cudaGetLastError();
-            std::memset(alpha, 0, count * sizeof(double));
-        }
-        return DG_OK;
-    }
+    if (!s->av) return zero_fill(s, alpha, count);
     int rc = copy_vars(s, alpha, 1, s->W0 + (size_t)s->Vc * s->ncells, s->V, 1);
     if (rc) return rc;
     CU(cudaStreamSynchronize(s->stream));
@@ -587,8 +610,8 @@ int dg_eval_rhs(dg_solver *s, double *out, size_t count, double *alpha_out, size
             rc = copy_vars(s, alpha_out, 1, s->WA + (size_t)s->Vc * s->ncells, s->V, 1);
             if (rc) return rc;
         } else {
-            CU(cudaStreamSynchronize(s->stream));
-            std::memset(alpha_out, 0, alpha_count * sizeof(double));
+            rc = zero_fill(s, alpha_out, alpha_count);
+            if (rc) return rc;
         }
     }
     return check_flag(s);
@@ -599,16 +622,28 @@ int dg_profile_stage(dg_solver *s, int reps, double *face_ms, double *stage_ms) 
     if (reps < 1) return fail(DG_EINVAL, "reps must be >= 1");
     DgStageArgs a;
     fill_args(s, &a);
-    a.w_prev = s->W0;
-    a.w_n = s->W0;
-    a.w_out = s->WA;
-    a.rhs_only = 1;
-    cudaEvent_t ev[3];
-    for (int i = 0; i < 3; ++i) CU(cudaEventCreate(&ev[i]));
+    if (s->opt.rk_stages >= 3) {
+        // the middle stage of SSP-RK3 with its real combine arguments (reads u^n and u^(i-1), writes u^(i)):
+        // u^(i-1) := a copy of the current state in WA, output to WB; W0 (the state) is not modified
+        CU(cudaMemcpyAsync(s->WA, s->W0, s->nstate * sizeof(double), cudaMemcpyDeviceToDevice, s->stream));
+        a.w_prev = s->WA;
+        a.w_n = s->W0;
+        a.w_out = s->WB;
+        a.rk_a = 0.75;
+        a.rk_b = 0.25;
+        a.rk_c = 0.25;
+    } else {
+        a.w_prev = s->W0;
+        a.w_n = s->W0;
+        a.w_out = s->WA;
+        a.rhs_only = 1;
+    }
+    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
+    cudaError_t e = cudaSuccess;
+    for (int i = 0; i < 3 && e == cudaSuccess; ++i) e = cudaEventCreate(&ev[i]);
     double tf = 0.0, ts = 0.0;
-    int rc = DG_OK;
-    for (int k = 0; k < reps + 1 && rc == DG_OK; ++k) {   // first pass is a warm-up
-        cudaError_t e = cudaEventRecord(ev[0], s->stream);
+    for (int k = 0; k < reps + 1 && e == cudaSuccess; ++k) {   // first pass is a warm-up
+        e = cudaEventRecord(ev[0], s->stream);
         if (e == cudaSuccess) e = s->fn.launch(s->visc, s->av, &a, s->stream, 2);
         if (e == cudaSuccess) e = cudaEventRecord(ev[1], s->stream);
         if (e == cudaSuccess) e = s->fn.launch(s->visc, s->av, &a, s->stream, 3);
@@ -617,15 +652,15 @@ int dg_profile_stage(dg_solver *s, int reps, double *face_ms, double *stage_ms) 
         float f = 0.f, g = 0.f;
         if (e == cudaSuccess) e = cudaEventElapsedTime(&f, ev[0], ev[1]);
         if (e == cudaSuccess) e = cudaEventElapsedTime(&g, ev[1], ev[2]);
-        if (e != cudaSuccess) rc = fail(DG_ECUDA, "dg_profile_stage: %s", cudaGetErrorString(e));
         s->launches += 2;
         if (k > 0) {
             tf += f;
             ts += g;
         }
     }
-    for (int i = 0; i < 3; ++i) cudaEventDestroy(ev[i]);
-    if (rc) return rc;
+    for (int i = 0; i < 3; ++i)
+        if (ev[i]) cudaEventDestroy(ev[i]);
+    if (e != cudaSuccess) return fail(DG_ECUDA, "dg_profile_stage: %s", cudaGetErrorString(e));
     if (face_ms) *face_ms = tf / reps;
     if (stage_ms) *stage_ms = ts / reps;
     return check_flag(s);
@@ -680,19 +715,24 @@ int dg_measure_fp64_peak(int iters, double *flops_per_s, void *cuda_stream) {
     double *d = nullptr;
     CU(cudaMalloc(&d, sizeof(double)));
     const int blocks = prop.multiProcessorCount * 8;
-    cudaEvent_t e0, e1;
-    CU(cudaEventCreate(&e0));
-    CU(cudaEventCreate(&e1));
-    dg_dfma_kernel<<<blocks, 256, 0, st>>>(d, iters / 4 + 1, 1.0, 0.0);
-    CU(cudaEventRecord(e0, st));
-    dg_dfma_kernel<<<blocks, 256, 0, st>>>(d, iters, 1.0, 0.0);
-    CU(cudaEventRecord(e1, st));
-    CU(cudaEventSynchronize(e1));
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
     float ms = 0.f;
-    CU(cudaEventElapsedTime(&ms, e0, e1));
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
+    cudaError_t e = cudaEventCreate(&e0);
+    if (e == cudaSuccess) e = cudaEventCreate(&e1);
+    if (e == cudaSuccess) {
+        dg_dfma_kernel<<<blocks, 256, 0, st>>>(d, iters / 4 + 1, 1.0, 0.0);
+        e = cudaEventRecord(e0, st);
+    }
+    if (e == cudaSuccess) {
+        dg_dfma_kernel<<<blocks, 256, 0, st>>>(d, iters, 1.0, 0.0);
+        e = cudaEventRecord(e1, st);
+    }
+    if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
     cudaFree(d);
+    if (e != cudaSuccess) return fail(DG_ECUDA, "dg_measure_fp64_peak: %s", cudaGetErrorString(e));
     const double flops = 2.0 * 64.0 * (double)iters * 256.0 * (double)blocks;
     *flops_per_s = flops / (ms * 1e-3);
     return DG_OK;

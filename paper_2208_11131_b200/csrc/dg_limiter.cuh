@@ -102,7 +102,7 @@ __global__ void __launch_bounds__(256, 2) dg_limiter_kernel(double *w, int V, in
         for (int b = 0; b < D; ++b) mm = fma(m[1 + b], m[1 + b], mm);
         const double pb = (gamma - 1.0) * (m[1 + D] - 0.5 * mm / m[0]);
         const bool ok = (m[0] > 0.0) && (pb > 0.0);
-        if (!ok && cell0 + tid < ncells) atomicOr(flag, 1);       // "a code crash is unavoidable"
+        if (!ok && cell0 + tid < ncells) atomicOr(flag, 8);       // "a code crash is unavoidable"
         act[tid] = (ok && cell0 + tid < ncells) ? 1 : 0;
         rbot[tid] = 1.0e-6 * m[0];
         pbot[tid] = 1.0e-6 * pb;

@@ -78,6 +78,16 @@ struct Cfg {
     static_assert(kSmemBytes <= kSmemMax, "per-cell footprint exceeds shared memory");
     // A tile of m x m points (the two fastest axes) is swept in registers when it fits (m <= 5).
     static constexpr bool BLK = (M >= 2) && (M * M <= 25);
+    // Format of the face-flux buffer.  PP (register-tile configurations, consumed by dg_stage2_kernel): the flux of
+    // face axis A is projected on the transverse modes of the axes BELOW A only -- x faces stay nodal, y faces are
+    // modal in x (nodal in z), z faces are modal in x and y -- because the stage kernel injects the lift of axis A
+    // right after its own projection sweep along A and the remaining sweeps finish the transverse projection.
+    // Otherwise (dg_stage_kernel): fully projected on both transverse axes.
+#ifdef DG_USE_V1
+    static constexpr bool PP = false;
+#else
+    static constexpr bool PP = BLK;
+#endif
 };
 
 // Shared-memory arrays are indexed by a flat point index P = slot*NPTS + p and the cell:  offset = at(P)*C + cell.
@@ -425,7 +435,7 @@ __device__ __forceinline__ void wavespeed_points(const double *RA, double gamma,
         cmax = (cs > cmax) ? cs : cmax;   // NaN-safe: NaN never becomes the maximum
         vmax = (vm > vmax) ? vm : vmax;
     }
-    if (bad) atomicOr(flag, 1);
+    if (bad) atomicOr(flag, 4);   // flag bits: 1 volume point, 2 face point, 4 wave-speed pass, 8 limiter (cell mean)
     block_max2<NT>(cmax, vmax, red, maxbits, tid);
 }
 
@@ -696,7 +706,7 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA
 #pragma unroll
             for (int v = 0; v < Vc; ++v) RX[LF::at2(oUL + v, k) * C + cell] = Fh[v];
         }
-        if (bad) atomicOr(p.flag, 1);
+        if (bad) atomicOr(p.flag, 2);
     }
     __syncthreads();
 
@@ -707,8 +717,8 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA
             const int cell = it % C, g = it / C;
             double t[M * M];
             tile_load<M, C, LF>(RX, oUL + g, cell, t);
-            tile_x<DG_SEL_VTG, M>(t);
-            tile_y<DG_SEL_VTG, M>(t);
+            if (!K::PP || A >= 1) tile_x<DG_SEL_VTG, M>(t);     // tile axes: the two transverse axes in increasing order
+            if (!K::PP || A >= 2) tile_y<DG_SEL_VTG, M>(t);
             if (cell0 + cell < p.ncells) {
 #pragma unroll
                 for (int q = 0; q < M * M; ++q) out[(size_t)(g * Nf + q) * p.ncells + cell0 + cell] = t[q];
@@ -735,7 +745,9 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA
 #pragma unroll
             for (int j = 0; j < M; ++j) {
                 double acc;
-                if (M > 1) {
+                if (K::PP && D == 2 && A == 0) {
+                    acc = in[j];                       // x faces stay nodal in y (see Cfg::PP)
+                } else if (M > 1) {
                     acc = c_tab.VtG[j * 8] * in[0];
 #pragma unroll
                     for (int i = 1; i < M; ++i) acc = fma(c_tab.VtG[j * 8 + i], in[i], acc);

@@ -2,6 +2,7 @@
 // (Euler, NS, AV, NS+AV) and exports plain launch functions for dg_api.cu.  Compiled 16 times by build.py
 // with -DDG_DIM=2|3 -DDG_M=1..8 (keeps ptxas work parallel and each image small).
 #include "dg_stage.cuh"
+#include "dg_stage2.cuh"
 #include "dg_limiter.cuh"
 #include "dg_dispatch.h"
 
@@ -18,6 +19,14 @@ cudaError_t configure() {
     cudaError_t e = cudaFuncSetAttribute(dgk::dg_stage_kernel<DG_DIM, DG_M, VISC, AV>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, K::kSmemBytes);
     if (e != cudaSuccess) return e;
+    // NB: a kernel template must only ever be instantiated in the translation unit of its own (dim, m): every unit
+    // has its own __constant__ tables, and the host stubs of equal instantiations are merged by the linker
+    if constexpr (K::PP) {
+        e = cudaFuncSetAttribute(dgk::dg_stage2_kernel<DG_DIM, DG_M, VISC, AV>,
+                                 cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 dgk::Cfg2<DG_DIM, DG_M, VISC, AV>::kSmemBytes);
+        if (e != cudaSuccess) return e;
+    }
     e = cudaFuncSetAttribute(dgk::dg_face_kernel<DG_DIM, DG_M, VISC, AV>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              dgk::FaceCfg<DG_DIM, DG_M, VISC, AV>::kSmemBytes);
     if (e != cudaSuccess) return e;
@@ -44,16 +53,32 @@ cudaError_t launch(const DgStageArgs &a, cudaStream_t st, int wavespeed_only) {
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
-    if (wavespeed_only != 2) dgk::dg_stage_kernel<DG_DIM, DG_M, VISC, AV><<<blocks, K::NT, K::kSmemBytes, st>>>(a);
+    if (wavespeed_only != 2) {
+        if constexpr (K::PP) {
+            // register-tile configurations (2 <= m <= 5): second-generation stage kernel (dg_stage2.cuh)
+            using K2 = dgk::Cfg2<DG_DIM, DG_M, VISC, AV>;
+            const int blocks2 = (a.ncells + K2::C - 1) / K2::C;
+            dgk::dg_stage2_kernel<DG_DIM, DG_M, VISC, AV><<<blocks2, K2::NT, K2::kSmemBytes, st>>>(a);
+        } else {
+            dgk::dg_stage_kernel<DG_DIM, DG_M, VISC, AV><<<blocks, K::NT, K::kSmemBytes, st>>>(a);
+        }
+    }
     return cudaGetLastError();
 }
 
 template <bool VISC, bool AV>
 void info(int *c, int *nt, int *smem) {
     using K = dgk::Cfg<DG_DIM, DG_M, VISC, AV>;
-    *c = K::C;
-    *nt = K::NT;
-    *smem = K::kSmemBytes;
+    if constexpr (K::PP) {
+        using K2 = dgk::Cfg2<DG_DIM, DG_M, VISC, AV>;
+        *c = K2::C;
+        *nt = K2::NT;
+        *smem = K2::kSmemBytes;
+    } else {
+        *c = K::C;
+        *nt = K::NT;
+        *smem = K::kSmemBytes;
+    }
 }
 
 }  // namespace

@@ -439,6 +439,26 @@ __device__ __forceinline__ void wavespeed_points(const double *RA, double gamma,
     block_max2<NT>(cmax, vmax, red, maxbits, tid);
 }
 
+// Block -> tile map.  A tile is C consecutive cells of one x-row.  In 3D the tiles are visited in groups of 8 y-rows
+// x 8 z-planes (x fastest, then y within the group, then z within the group), so that the y and z neighbours of a
+// tile are at most 8 x-rows away in launch order and their rows (state for the face kernel, face fluxes for the
+// stage kernel) are still in L2 -- or in flight -- when they are read; 1/8 of the tiles per axis reach across a
+// group boundary.  Falls back to the natural order when the mesh does not divide (nx % C, ny % 8, nz % 8).
+template <int D, int C>
+__device__ __forceinline__ int tile_of_block(int b, int nx, int ny, int nz) {
+    if (D != 3 || (nx % C) != 0 || (ny % 8) != 0 || (nz % 8) != 0) return b;
+    const int ntx = nx / C;
+    const int gsz = ntx * 64;
+    const int gi = b / gsz;
+    int r = b - gi * gsz;
+    const int xb = r % ntx;
+    r /= ntx;
+    const int ngy = ny / 8;
+    const int iy = (gi % ngy) * 8 + (r % 8);
+    const int iz = (gi / ngy) * 8 + (r / 8);
+    return (iz * ny + iy) * ntx + xb;
+}
+
 // address of row `row` (compile-time multiple after unrolling) of a [row][cell] global array: one IMAD.WIDE
 __device__ __forceinline__ const double *row_ptr(const double *base, unsigned row, unsigned ncells) {
     return base + (unsigned long long)row * ncells;
@@ -772,7 +792,7 @@ __global__ void __launch_bounds__(DG_FACE_NT, DG_FACE_MINB) dg_face_kernel(const
     int *nbr = reinterpret_cast<int *>(RX + K::NQ * K::Nf * C);
     double *bar = RX + K::NQ * K::Nf * C + (D * C + 1) / 2;   // mbarrier of the bulk copies, after nbr[D*C]
     const int tid = threadIdx.x;
-    const int cell0 = blockIdx.x * C;
+    const int cell0 = tile_of_block<D, C>(blockIdx.x, p.nx, p.ny, p.nz) * C;
     const bool bulk = bulk_ok<C>(cell0, p.ncells);
     if (bulk) {
         if (tid == 0) mbar_init(bar, 1);

@@ -5,16 +5,18 @@
 //     values in y,z), y faces after P_y (modal in x, nodal in z), z faces after P_z (modal in x,y) -- and the stage
 //     combine writes straight to global memory;
 //   * the own modes read from global memory directly into the register tiles of the first two expansion sweeps;
-//   * six barrier-separated phases in 3D (three in 2D) instead of twelve, ~40 % fewer shared-memory wavefronts, and
-//     a per-cell footprint of (V + D*Vc) m^D doubles, which lets two blocks share an SM.
-// The face kernel writes the face fluxes in the matching partially projected form (DG_FLUX_PARTIAL in dg_stage.cuh).
+//   * six barrier-separated phases in 3D (three in 2D) instead of twelve, ~35 % fewer shared-memory wavefronts, and
+//     a per-cell footprint of (V + D*Vc) m^D doubles;
+//   * the global inputs of the later phases (face fluxes, u^n, u^(i-1)) are requested before the barrier in front of
+//     the phase that needs them, so that one memory round trip covers a thread's items and overlaps the barrier wait;
+//   * blocks walk the mesh in (y,z)-blocked order (tile_of_block) so that the lower y and z neighbours' face fluxes
+//     are still in L2 when they are read.
+// The face kernel writes the face fluxes in the matching partially projected form (Cfg::PP in dg_stage.cuh).
+// Measured dead ends (profiles/r2_stage_experiments.md): persistent blocks with the next tile's modes staged by TMA
+// tensor copies, L2 prefetch hints, 12 warps per block -- all slower than this form.
 #pragma once
 
 #include "dg_stage.cuh"
-
-#ifndef DG_S2_NT
-#define DG_S2_NT 256
-#endif
 
 namespace dgk {
 
@@ -22,33 +24,27 @@ template <int D, int M, bool VISC, bool AV>
 struct Cfg2 {
     using K = Cfg<D, M, VISC, AV>;
     static constexpr int V = K::V, Vc = K::Vc, Np = K::Np, Nf = K::Nf;
-    static constexpr int NT = DG_S2_NT;
-    static constexpr int FP = V * Np + D * Vc * Np;                  // doubles per cell: U + GR
+    // one block of 16 warps per SM in 3D (measured: 128-byte rows of 16 cells beat two blocks of 8 cells at 128^3);
+    // 2D tiles are small, several 8-warp blocks share an SM
+    static constexpr int NT = (D == 3) ? 512 : 256;
+    static constexpr int CMAX = (D == 3 && M >= 4) ? 16 : 32;
+    // doubles per cell: U (nodal values) + GR (gradients -> fluxes)
+    static constexpr int FP = V * Np + D * Vc * Np;
     // Wk[c], wave-speed scratch, sensor partials, S table
     static constexpr int extra_doubles(int c) { return c + 2 * (NT / 32) + (AV ? 4 * (NT / 32) * c : 0) + M * M + 2; }
-    static constexpr int fit(int budget) {
-        int c = 32;
-        while (c > 1 && (c * FP + extra_doubles(c)) * 8 > budget) c >>= 1;
+    static constexpr int pick_c() {
+        int c = CMAX;
+        while (c > 1 && (c * FP + extra_doubles(c)) * 8 > 227 * 1024 - 1024) c >>= 1;
         return c;
     }
-    // two resident blocks per SM when at least 8 cells fit half the shared memory, else one block
-    static constexpr int C2 = fit((227 * 1024) / 2 - 1024);
-    static constexpr int C1 = fit(227 * 1024 - 1024);
-    static constexpr int MINB = (C2 >= 8) ? 2 : 1;
-    static constexpr int C = (C2 >= 8) ? C2 : C1;
+    static constexpr int C = pick_c();
     static constexpr int kSmemBytes = (C * FP + extra_doubles(C)) * 8;
     static_assert(kSmemBytes <= kSmemMax, "stage kernel 2: per-cell footprint exceeds shared memory");
     static_assert(NT % C == 0, "threads per block must be a multiple of cells per block");
 };
 
-// u^(i) = a u^n + b u^(i-1) + c dt L, SSPRK(5,4) auxiliary row, shock-sensor sums (Eq. 42)
-struct CombineCtx {
-    double cdt, auxc;
-    bool need_n, need_p, rhs_only, active, sensor, aux;
-};
-
 template <int D, int M, bool VISC, bool AV>
-__global__ void __launch_bounds__(DG_S2_NT, (Cfg2<D, M, VISC, AV>::MINB)) dg_stage2_kernel(const DgStageArgs p) {
+__global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), 1) dg_stage2_kernel(const DgStageArgs p) {
     using K = Cfg<D, M, VISC, AV>;
     using K2 = Cfg2<D, M, VISC, AV>;
     constexpr int C = K2::C, NT = K2::NT, V = K::V, Vc = K::Vc, Np = K::Np, Nf = K::Nf;
@@ -64,89 +60,48 @@ __global__ void __launch_bounds__(DG_S2_NT, (Cfg2<D, M, VISC, AV>::MINB)) dg_sta
     double *sens = red + 2 * (NT / 32);           // [4][NT/32][C] partial sensor sums (AV only)
     double *sS = sens + (AV ? 4 * (NT / 32) * C : 0);   // weak-derivative matrix S for run-time row indices
     const int tid = threadIdx.x;
-    const int cell0 = blockIdx.x * C;
     const int cl = tid % C;
-    const int cg = min(cell0 + cl, p.ncells - 1);
-    const bool active = cell0 + cl < p.ncells;
-    int nbm[D];                                   // lower neighbour along each axis (periodic wrap)
-    {
-        const int ix = cg % p.nx;
-        const int iy = (cg / p.nx) % p.ny;
-        const int iz = cg / (p.nx * p.ny);
-        nbm[0] = cg + ((ix == 0) ? p.nx - 1 : -1);
-        nbm[1] = cg + ((iy == 0) ? (p.ny - 1) * p.nx : -p.nx);
-        if (D == 3) nbm[D - 1] = cg + ((iz == 0) ? (p.nz - 1) * p.nx * p.ny : -p.nx * p.ny);
-    }
     const double ih = 1.0 / p.h;
     const double pref = (D == 3 ? 0.25 : 0.5) * ih;
+    const double cdt = p.rhs_only ? 1.0 : p.rk_c * p.scal[0];
+    const bool need_n = !p.rhs_only, need_p = !p.rhs_only && p.rk_b != 0.0;
+    const bool has_aux = p.w_aux != nullptr;
     if (tid < MM) sS[tid] = c_tab.S[(tid / M) * 8 + tid % M];
-    if (AV && tid < C) {
-        // wiggle source of Eq. 45 from the previous step's sensor (readings A14, A15)
-        const int c = min(cell0 + tid, p.ncells - 1);
-        const double S = p.sens_prev[c];
-        const double G = p.sens_prev[p.ncells + c];
-        Wk[tid] = (S > p.s_onset) ? p.f_w * fmax(0.0, G) : 0.0;
-    }
+    {
+        const int tile = tile_of_block<D, C>(blockIdx.x, p.nx, p.ny, p.nz);
+        const int cell0 = tile * C;
+        const int cg = min(cell0 + cl, p.ncells - 1);
+        const bool active = cell0 + cl < p.ncells;
+        int nbm[D];                               // lower neighbour along each axis (periodic wrap)
+        {
+            const int ix = cg % p.nx;
+            const int iy = (cg / p.nx) % p.ny;
+            const int iz = cg / (p.nx * p.ny);
+            nbm[0] = cg + ((ix == 0) ? p.nx - 1 : -1);
+            nbm[1] = cg + ((iy == 0) ? (p.ny - 1) * p.nx : -p.nx);
+            if (D == 3) nbm[D - 1] = cg + ((iz == 0) ? (p.nz - 1) * p.nx * p.ny : -p.nx * p.ny);
+        }
+        if (AV && tid < C) {
+            // wiggle source of Eq. 45 from the previous step's sensor (readings A14, A15)
+            const int c = min(cell0 + tid, p.ncells - 1);
+            const double S = p.sens_prev[c];
+            const double G = p.sens_prev[p.ncells + c];
+            Wk[tid] = (S > p.s_onset) ? p.f_w * fmax(0.0, G) : 0.0;
+        }
 
-    // ---- A: own modes, global -> register tile; expansion along x and y (Eq. 21) ----
-    for (int it = tid; it < V * NTILE * C; it += NT) {
-        const int g = it / C;                     // v*NTILE + lz
-        const int v = g / NTILE, lz = g % NTILE;
-        const double *src = p.w_prev + (size_t)(lz * MM * V + v) * p.ncells + cg;
-        double t[MM];
+        // ---- A: own modes, global -> register tile; expansion along x and y (Eq. 21) ----
+        for (int it = tid; it < V * NTILE * C; it += NT) {
+            const int g = it / C;                 // v*NTILE + lz
+            const int v = g / NTILE, lz = g % NTILE;
+            double t[MM];
+            const double *src = p.w_prev + (size_t)(lz * MM * V + v) * p.ncells + cg;
 #pragma unroll
-        for (int q = 0; q < MM; ++q) t[q] = __ldg(row_ptr(src, q * V, p.ncells));
-        tile_x<DG_SEL_V, M>(t);
-        tile_y<DG_SEL_V, M>(t);
-        tile_store<M, C, L>(U, g, cl, t);
-        if (D == 2 && GRAD && v < Vc) {
-            double a[MM];
-#pragma unroll
-            for (int q = 0; q < MM; ++q) a[q] = t[q];
-            tile_x<DG_SEL_DHAT, M>(a);
-#pragma unroll
-            for (int q = 0; q < MM; ++q) a[q] *= 2.0 * ih;
-            tile_store<M, C, L>(GR, g, cl, a);
-            tile_y<DG_SEL_DHAT, M>(t);
-#pragma unroll
-            for (int q = 0; q < MM; ++q) t[q] *= 2.0 * ih;
-            tile_store<M, C, L>(GR, Vc * NTILE + g, cl, t);
-        }
-    }
-    __syncthreads();
-    if (D == 3) {
-        // ---- B: expansion along z, z derivative ----
-        for (int it = tid; it < V * MM * C; it += NT) {
-            const int r = it / C;
-            const int q = r % MM, v = r / MM;
-            double in[M], u[M];
-#pragma unroll
-            for (int l = 0; l < M; ++l) in[l] = U[L::at2(v, q + l * MM) * C + cl];
-#pragma unroll
-            for (int j = 0; j < M; ++j) {
-                double acc = c_tab.V[j * 8] * in[0];
-#pragma unroll
-                for (int l = 1; l < M; ++l) acc = fma(c_tab.V[j * 8 + l], in[l], acc);
-                u[j] = acc;
-                U[L::at2(v, q + j * MM) * C + cl] = acc;
-            }
-            if (GRAD && v < Vc) {
-#pragma unroll
-                for (int j = 0; j < M; ++j) {
-                    double acc = c_tab.Dhat[j * 8] * u[0];
-#pragma unroll
-                    for (int i = 1; i < M; ++i) acc = fma(c_tab.Dhat[j * 8 + i], u[i], acc);
-                    GR[L::at2(2 * Vc + v, q + j * MM) * C + cl] = acc * (2.0 * ih);
-                }
-            }
-        }
-        __syncthreads();
-        if (GRAD) {
-            // ---- D: x and y derivatives of the nodal values, one tile load for both ----
-            for (int it = tid; it < Vc * NTILE * C; it += NT) {
-                const int g = it / C;
-                double t[MM], a[MM];
-                tile_load<M, C, L>(U, g, cl, t);
+            for (int q = 0; q < MM; ++q) t[q] = __ldg(row_ptr(src, q * V, p.ncells));
+            tile_x<DG_SEL_V, M>(t);
+            tile_y<DG_SEL_V, M>(t);
+            tile_store<M, C, L>(U, g, cl, t);
+            if (D == 2 && GRAD && v < Vc) {
+                double a[MM];
 #pragma unroll
                 for (int q = 0; q < MM; ++q) a[q] = t[q];
                 tile_x<DG_SEL_DHAT, M>(a);
@@ -158,242 +113,311 @@ __global__ void __launch_bounds__(DG_S2_NT, (Cfg2<D, M, VISC, AV>::MINB)) dg_sta
                 for (int q = 0; q < MM; ++q) t[q] *= 2.0 * ih;
                 tile_store<M, C, L>(GR, Vc * NTILE + g, cl, t);
             }
-            __syncthreads();
         }
-    }
-    {
-        // ---- E: point-wise fluxes G_a = f_a - F_NS,a - eps d_a u (Eq. 24; 315 Eq. 38), alpha source ----
-        bool bad = false;
-        const double decay = (double)M / (p.f_tau * p.h);      // 1/tau = (n+1) c_s / (f_tau h), Eq. 44
-        for (int it = tid; it < Np * C; it += NT) {
-            const int j = it / C;
-            double u[Vc];
+        __syncthreads();
+        if (D == 3) {
+            // ---- B: expansion along z, z derivative ----
+            for (int it = tid; it < V * MM * C; it += NT) {
+                const int r = it / C;
+                const int q = r % MM, v = r / MM;
+                double in[M], u[M];
 #pragma unroll
-            for (int v = 0; v < Vc; ++v) u[v] = U[L::at2(v, j) * C + cl];
-            const Prim<D> q = primitives<D>(u, p.gamma);
-            bad |= !(q.rho > 0.0) || !(q.p > 0.0);
-            double g[D][D + 2], dv[D][D];
-            double divv = 0.0, eps = 0.0;
+                for (int l = 0; l < M; ++l) in[l] = U[L::at2(v, q + l * MM) * C + cl];
+#pragma unroll
+                for (int j = 0; j < M; ++j) {
+                    double acc = c_tab.V[j * 8] * in[0];
+#pragma unroll
+                    for (int l = 1; l < M; ++l) acc = fma(c_tab.V[j * 8 + l], in[l], acc);
+                    u[j] = acc;
+                    U[L::at2(v, q + j * MM) * C + cl] = acc;
+                }
+                if (GRAD && v < Vc) {
+#pragma unroll
+                    for (int j = 0; j < M; ++j) {
+                        double acc = c_tab.Dhat[j * 8] * u[0];
+#pragma unroll
+                        for (int i = 1; i < M; ++i) acc = fma(c_tab.Dhat[j * 8 + i], u[i], acc);
+                        GR[L::at2(2 * Vc + v, q + j * MM) * C + cl] = acc * (2.0 * ih);
+                    }
+                }
+            }
+            __syncthreads();
             if (GRAD) {
+                // ---- D: x and y derivatives of the nodal values, one tile load for both ----
+                for (int it = tid; it < Vc * NTILE * C; it += NT) {
+                    const int g = it / C;
+                    double t[MM], a[MM];
+                    tile_load<M, C, L>(U, g, cl, t);
 #pragma unroll
-                for (int b = 0; b < D; ++b)
+                    for (int q = 0; q < MM; ++q) a[q] = t[q];
+                    tile_x<DG_SEL_DHAT, M>(a);
 #pragma unroll
-                    for (int v = 0; v < Vc; ++v) g[b][v] = GR[L::at2(b * Vc + v, j) * C + cl];
-                velocity_gradient<D>(q, g, dv);
+                    for (int q = 0; q < MM; ++q) a[q] *= 2.0 * ih;
+                    tile_store<M, C, L>(GR, g, cl, a);
+                    tile_y<DG_SEL_DHAT, M>(t);
 #pragma unroll
-                for (int b = 0; b < D; ++b) divv += dv[b][b];
+                    for (int q = 0; q < MM; ++q) t[q] *= 2.0 * ih;
+                    tile_store<M, C, L>(GR, Vc * NTILE + g, cl, t);
+                }
+                __syncthreads();
             }
-            if (AV) {
-                const double al = U[L::at2(Vc, j) * C + cl];
-                const double cs = fast_sqrt(p.gamma * q.p * q.ir);
-                eps = fmin(fmax(al, 0.0), p.alpha_max) * cs * (p.h / (double)M);        // Eq. 46, A17
-                // Eq. 43-45: shock source + wiggle source - decay; stored pre-scaled by h/2 for the projection
-                const double src = p.f_v * fmax(0.0, -divv) + Wk[cl] - al * (cs * decay);
-                U[L::at2(Vc, j) * C + cl] = 0.5 * p.h * src;
-            }
+        }
+        {
+            // ---- E: point-wise fluxes G_a = f_a - F_NS,a - eps d_a u (Eq. 24; 315 Eq. 38), alpha source ----
+            bool bad = false;
+            const double decay = (double)M / (p.f_tau * p.h);      // 1/tau = (n+1) c_s / (f_tau h), Eq. 44
+            for (int it = tid; it < Np * C; it += NT) {
+                const int j = it / C;
+                double u[Vc];
 #pragma unroll
-            for (int a = 0; a < D; ++a) {
-                double F[Vc];
-                euler_flux<D>(u, q, a, F);
-                if (VISC) ns_flux_sub<D>(q, g, dv, divv, a, p.gamma, p.nu, p.chi, F);
+                for (int v = 0; v < Vc; ++v) u[v] = U[L::at2(v, j) * C + cl];
+                const Prim<D> q = primitives<D>(u, p.gamma);
+                bad |= !(q.rho > 0.0) || !(q.p > 0.0);
+                double g[D][D + 2], dv[D][D];
+                double divv = 0.0, eps = 0.0;
+                if (GRAD) {
+#pragma unroll
+                    for (int b = 0; b < D; ++b)
+#pragma unroll
+                        for (int v = 0; v < Vc; ++v) g[b][v] = GR[L::at2(b * Vc + v, j) * C + cl];
+                    velocity_gradient<D>(q, g, dv);
+#pragma unroll
+                    for (int b = 0; b < D; ++b) divv += dv[b][b];
+                }
                 if (AV) {
-#pragma unroll
-                    for (int v = 0; v < Vc; ++v) F[v] -= eps * g[a][v];
+                    const double al = U[L::at2(Vc, j) * C + cl];
+                    const double cs = fast_sqrt(p.gamma * q.p * q.ir);
+                    eps = fmin(fmax(al, 0.0), p.alpha_max) * cs * (p.h / (double)M);        // Eq. 46, A17
+                    // Eq. 43-45: shock source + wiggle source - decay; stored pre-scaled by h/2 for the projection
+                    const double src = p.f_v * fmax(0.0, -divv) + Wk[cl] - al * (cs * decay);
+                    U[L::at2(Vc, j) * C + cl] = 0.5 * p.h * src;
                 }
 #pragma unroll
-                for (int v = 0; v < Vc; ++v) GR[L::at2(a * Vc + v, j) * C + cl] = F[v];
+                for (int a = 0; a < D; ++a) {
+                    double F[Vc];
+                    euler_flux<D>(u, q, a, F);
+                    if (VISC) ns_flux_sub<D>(q, g, dv, divv, a, p.gamma, p.nu, p.chi, F);
+                    if (AV) {
+#pragma unroll
+                        for (int v = 0; v < Vc; ++v) F[v] -= eps * g[a][v];
+                    }
+#pragma unroll
+                    for (int v = 0; v < Vc; ++v) GR[L::at2(a * Vc + v, j) * C + cl] = F[v];
+                }
             }
+            if (bad) atomicOr(p.flag, 1);
         }
-        if (bad) atomicOr(p.flag, 1);
-    }
-    __syncthreads();
-
-    // stage combine of one modal value and the sensor sums of Eq. 42 (readings A13/A15)
-    const double cdt = p.rhs_only ? 1.0 : p.rk_c * p.scal[0];
-    const bool need_n = !p.rhs_only, need_p = !p.rhs_only && p.rk_b != 0.0;
-    const bool has_aux = p.w_aux != nullptr;
-    double sA = 0.0, sB = 0.0, dA = 0.0, dB = 0.0;
-
-    // ---- G: weak-form derivative N = sum_a S_a G_a, projection along x and y, lift of the x and y faces ----
-    for (int it = tid; it < V * NTILE * C; it += NT) {
-        const int g = it / C;                     // v*NTILE + jz
-        const int v = g / NTILE, jz = g % NTILE;
-        double n[MM];
-        if (v < Vc) {
-            // face fluxes of this tile: x faces as nodal values (jy, jz), y faces modal in x, nodal in z
-            double fxp[M], fxm[M], fyp[M], fym[M];
-            {
+        // face fluxes of this thread's G items, requested before the barrier: x faces as nodal values (jy, jz), y faces
+        // modal in x and nodal in z (Cfg::PP); own cell = upper face, lower neighbour's = lower face
+        constexpr int NKG = (V * NTILE * C + NT - 1) / NT;
+        double gf[NKG][4][M];
+#pragma unroll
+        for (int k = 0; k < NKG; ++k) {
+            const int g = (tid + k * NT) / C;     // v*NTILE + jz
+            const int v = g / NTILE, jz = g % NTILE;
+#pragma unroll
+            for (int i = 0; i < M; ++i) gf[k][0][i] = gf[k][1][i] = gf[k][2][i] = gf[k][3][i] = 0.0;
+            if (g < Vc * NTILE) {
                 const double *fx = p.flux + (size_t)((0 * Vc + v) * Nf + jz * M) * p.ncells;
                 const double *fy = p.flux + (size_t)((1 * Vc + v) * Nf + jz * M) * p.ncells;
 #pragma unroll
-                for (int k = 0; k < M; ++k) {
-                    fxp[k] = __ldg(row_ptr(fx, k, p.ncells) + cg);
-                    fxm[k] = __ldg(row_ptr(fx, k, p.ncells) + nbm[0]);
-                    fyp[k] = __ldg(row_ptr(fy, k, p.ncells) + cg);
-                    fym[k] = __ldg(row_ptr(fy, k, p.ncells) + nbm[1]);
+                for (int i = 0; i < M; ++i) {
+                    gf[k][0][i] = __ldg(row_ptr(fx, i, p.ncells) + cg);
+                    gf[k][1][i] = __ldg(row_ptr(fx, i, p.ncells) + nbm[0]);
+                    gf[k][2][i] = __ldg(row_ptr(fy, i, p.ncells) + cg);
+                    gf[k][3][i] = __ldg(row_ptr(fy, i, p.ncells) + nbm[1]);
                 }
             }
-            double b[MM];
-            tile_load<M, C, L>(GR, (0 * Vc + v) * NTILE + jz, cl, n);
-            tile_x<DG_SEL_S, M>(n);
-            tile_load<M, C, L>(GR, (1 * Vc + v) * NTILE + jz, cl, b);
-            tile_y<DG_SEL_S, M>(b);
+        }
+        __syncthreads();
+
+        double sA = 0.0, sB = 0.0, dA = 0.0, dB = 0.0;      // shock-sensor sums of Eq. 42 (readings A13/A15)
+
+        // ---- G: weak-form derivative N = sum_a S_a G_a, projection along x and y, lift of the x and y faces ----
 #pragma unroll
-            for (int q = 0; q < MM; ++q) n[q] += b[q];
+        for (int k = 0; k < NKG; ++k) {
+            const int g = (tid + k * NT) / C;     // v*NTILE + jz
+            if (g >= V * NTILE) break;
+            const int v = g / NTILE, jz = g % NTILE;
+            double n[MM];
+            if (v < Vc) {
+                double b[MM];
+                tile_load<M, C, L>(GR, (0 * Vc + v) * NTILE + jz, cl, n);
+                tile_x<DG_SEL_S, M>(n);
+                tile_load<M, C, L>(GR, (1 * Vc + v) * NTILE + jz, cl, b);
+                tile_y<DG_SEL_S, M>(b);
+#pragma unroll
+                for (int q = 0; q < MM; ++q) n[q] += b[q];
+                if (D == 3) {
+#pragma unroll
+                    for (int kk = 0; kk < NTILE; ++kk) {
+                        tile_load<M, C, L>(GR, (2 * Vc + v) * NTILE + kk, cl, b);
+                        const double s = sS[jz * M + kk];
+#pragma unroll
+                        for (int q = 0; q < MM; ++q) n[q] = fma(s, b[q], n[q]);
+                    }
+                }
+                tile_x<DG_SEL_VTG, M>(n);
+#pragma unroll
+                for (int y = 0; y < M; ++y)
+#pragma unroll
+                    for (int x = 0; x < M; ++x)
+                        n[y * M + x] += c_tab.Pend[0][x] * gf[k][1][y] - c_tab.Pend[1][x] * gf[k][0][y];
+                tile_y<DG_SEL_VTG, M>(n);
+#pragma unroll
+                for (int y = 0; y < M; ++y)
+#pragma unroll
+                    for (int x = 0; x < M; ++x)
+                        n[y * M + x] += c_tab.Pend[0][y] * gf[k][3][x] - c_tab.Pend[1][y] * gf[k][2][x];
+            } else {
+                tile_load<M, C, L>(U, g, cl, n);      // alpha source (slot Vc of U)
+                tile_x<DG_SEL_VTG, M>(n);
+                tile_y<DG_SEL_VTG, M>(n);
+            }
             if (D == 3) {
+                tile_store<M, C, L>(U, g, cl, n);
+            } else {
+                // 2D: dw/dt of this (cell, variable) is complete: stage combine from registers
+                const double *bn = p.w_n + (size_t)v * p.ncells + cg;
+                const double *bp = p.w_prev + (size_t)v * p.ncells + cg;
+                double *bo = p.w_out + (size_t)v * p.ncells + cg;
+                double wn[MM], wp[MM];
 #pragma unroll
-                for (int k = 0; k < NTILE; ++k) {
-                    tile_load<M, C, L>(GR, (2 * Vc + v) * NTILE + k, cl, b);
-                    const double s = sS[jz * M + k];
+                for (int q = 0; q < MM; ++q) {
+                    wn[q] = need_n ? *row_ptr(bn, q * V, p.ncells) : 0.0;
+                    wp[q] = need_p ? __ldg(row_ptr(bp, q * V, p.ncells)) : 0.0;
+                }
 #pragma unroll
-                    for (int q = 0; q < MM; ++q) n[q] = fma(s, b[q], n[q]);
+                for (int q = 0; q < MM; ++q) {
+                    const double Ld = pref * n[q];
+                    double wnew = Ld;
+                    if (!p.rhs_only) wnew = fma(cdt, Ld, fma(p.rk_b, wp[q], p.rk_a * wn[q]));
+                    if (active) *row_ptr(bo, q * V, p.ncells) = wnew;
+                    if (has_aux && active) {
+                        const size_t gi = (size_t)(q * V + v) * p.ncells + cg;
+                        p.w_aux[gi] = fma(p.aux_c * p.scal[0], Ld, fma(p.aux_b, wp[q], p.aux_a * p.w_aux_in[gi]));
+                    }
+                    if (AV && p.do_sensor && v == 0) {
+                        const bool top = (q % M == M - 1) || (q / M == M - 1);
+                        sB = fma(wn[q], wn[q], sB);
+                        dB = fma(wn[q], Ld, dB);
+                        if (top) {
+                            sA = fma(wn[q], wn[q], sA);
+                            dA = fma(wn[q], Ld, dA);
+                        }
+                    }
+                    n[q] = wnew;
+                }
+                if (p.do_wavespeed && v < Vc) {
+                    tile_x<DG_SEL_V, M>(n);
+                    tile_y<DG_SEL_V, M>(n);
+                    tile_store<M, C, L>(U, g, cl, n);
                 }
             }
-            tile_x<DG_SEL_VTG, M>(n);
-#pragma unroll
-            for (int y = 0; y < M; ++y)
-#pragma unroll
-                for (int x = 0; x < M; ++x)
-                    n[y * M + x] += c_tab.Pend[0][x] * fxm[y] - c_tab.Pend[1][x] * fxp[y];
-            tile_y<DG_SEL_VTG, M>(n);
-#pragma unroll
-            for (int y = 0; y < M; ++y)
-#pragma unroll
-                for (int x = 0; x < M; ++x)
-                    n[y * M + x] += c_tab.Pend[0][y] * fym[x] - c_tab.Pend[1][y] * fyp[x];
-        } else {
-            tile_load<M, C, L>(U, g, cl, n);      // alpha source (slot Vc of U)
-            tile_x<DG_SEL_VTG, M>(n);
-            tile_y<DG_SEL_VTG, M>(n);
         }
         if (D == 3) {
-            tile_store<M, C, L>(U, g, cl, n);
-        } else {
-            // 2D: dw/dt of this (cell, variable) is complete: stage combine from registers
-            const double *bn = p.w_n + (size_t)v * p.ncells + cg;
-            const double *bp = p.w_prev + (size_t)v * p.ncells + cg;
-            double *bo = p.w_out + (size_t)v * p.ncells + cg;
-            double wn[MM], wp[MM];
+            // ---- H: projection along z, lift of the z faces, stage combine straight to global memory ----
+            // every global input of this thread's items (u^n, u^(i-1), the two z-face fluxes) is requested before the
+            // barrier, so that one memory round trip covers them all and overlaps the wait for the other warps
+            constexpr int NKH = (V * MM * C + NT - 1) / NT;
+            double hwn[NKH][M], hwp[NKH][M], hfz[NKH][2];
 #pragma unroll
-            for (int q = 0; q < MM; ++q) {
-                wn[q] = need_n ? *row_ptr(bn, q * V, p.ncells) : 0.0;
-                wp[q] = need_p ? __ldg(row_ptr(bp, q * V, p.ncells)) : 0.0;
-            }
+            for (int k = 0; k < NKH; ++k) {
+                const int r = (tid + k * NT) / C;
+                const int q = r % MM, v = r / MM;     // q = ly*M + lx
+                hfz[k][0] = hfz[k][1] = 0.0;
 #pragma unroll
-            for (int q = 0; q < MM; ++q) {
-                const double Ld = pref * n[q];
-                double wnew = Ld;
-                if (!p.rhs_only) wnew = fma(cdt, Ld, fma(p.rk_b, wp[q], p.rk_a * wn[q]));
-                if (active) *row_ptr(bo, q * V, p.ncells) = wnew;
-                if (has_aux && active) {
-                    const size_t gi = (size_t)(q * V + v) * p.ncells + cg;
-                    p.w_aux[gi] = fma(p.aux_c * p.scal[0], Ld, fma(p.aux_b, wp[q], p.aux_a * p.w_aux_in[gi]));
-                }
-                if (AV && p.do_sensor && v == 0) {
-                    const bool top = (q % M == M - 1) || (q / M == M - 1);
-                    sB = fma(wn[q], wn[q], sB);
-                    dB = fma(wn[q], Ld, dB);
-                    if (top) {
-                        sA = fma(wn[q], wn[q], sA);
-                        dA = fma(wn[q], Ld, dA);
+                for (int l = 0; l < M; ++l) hwn[k][l] = hwp[k][l] = 0.0;
+                if (r < V * MM) {
+                    if (v < Vc) {
+                        const double *fz = p.flux + (size_t)((2 * Vc + v) * Nf + q) * p.ncells;
+                        hfz[k][0] = __ldg(fz + cg);
+                        hfz[k][1] = __ldg(fz + nbm[D - 1]);
+                    }
+                    const double *bn = p.w_n + (size_t)(q * V + v) * p.ncells + cg;
+                    const double *bp = p.w_prev + (size_t)(q * V + v) * p.ncells + cg;
+#pragma unroll
+                    for (int l = 0; l < M; ++l) {
+                        if (need_n) hwn[k][l] = *row_ptr(bn, l * MM * V, p.ncells);
+                        if (need_p) hwp[k][l] = __ldg(row_ptr(bp, l * MM * V, p.ncells));
                     }
                 }
-                n[q] = wnew;
             }
-            if (p.do_wavespeed && v < Vc) {
-                tile_x<DG_SEL_V, M>(n);
-                tile_y<DG_SEL_V, M>(n);
-                tile_store<M, C, L>(U, g, cl, n);
-            }
-        }
-    }
-    if (D == 3) {
-        __syncthreads();
-        // ---- H: projection along z, lift of the z faces, stage combine straight to global memory ----
-        for (int it = tid; it < V * MM * C; it += NT) {
-            const int r = it / C;
-            const int q = r % MM, v = r / MM;     // q = ly*M + lx
-            double fzp = 0.0, fzm = 0.0;
-            if (v < Vc) {
-                const double *fz = p.flux + (size_t)((2 * Vc + v) * Nf + q) * p.ncells;
-                fzp = __ldg(fz + cg);
-                fzm = __ldg(fz + nbm[D - 1]);
-            }
-            const double *bn = p.w_n + (size_t)(q * V + v) * p.ncells + cg;
-            const double *bp = p.w_prev + (size_t)(q * V + v) * p.ncells + cg;
-            double *bo = p.w_out + (size_t)(q * V + v) * p.ncells + cg;
-            double wn[M], wp[M], in[M];
+            __syncthreads();
 #pragma unroll
-            for (int l = 0; l < M; ++l) {
-                wn[l] = need_n ? *row_ptr(bn, l * MM * V, p.ncells) : 0.0;
-                wp[l] = need_p ? __ldg(row_ptr(bp, l * MM * V, p.ncells)) : 0.0;
-            }
+            for (int k = 0; k < NKH; ++k) {
+                const int r = (tid + k * NT) / C;
+                if (r >= V * MM) break;
+                const int q = r % MM, v = r / MM;
+                double *bo = p.w_out + (size_t)(q * V + v) * p.ncells + cg;
+                double in[M];
 #pragma unroll
-            for (int j = 0; j < M; ++j) in[j] = U[L::at2(v, q + j * MM) * C + cl];
-            const bool topxy = (q % M == M - 1) || (q / M == M - 1);
+                for (int j = 0; j < M; ++j) in[j] = U[L::at2(v, q + j * MM) * C + cl];
+                const bool topxy = (q % M == M - 1) || (q / M == M - 1);
 #pragma unroll
-            for (int l = 0; l < M; ++l) {
-                double acc = c_tab.VtG[l * 8] * in[0];
+                for (int l = 0; l < M; ++l) {
+                    double acc = c_tab.VtG[l * 8] * in[0];
 #pragma unroll
-                for (int j = 1; j < M; ++j) acc = fma(c_tab.VtG[l * 8 + j], in[j], acc);
-                if (v < Vc) acc += c_tab.Pend[0][l] * fzm - c_tab.Pend[1][l] * fzp;
-                const double Ld = pref * acc;
-                double wnew = Ld;
-                if (!p.rhs_only) wnew = fma(cdt, Ld, fma(p.rk_b, wp[l], p.rk_a * wn[l]));
-                if (active) *row_ptr(bo, l * MM * V, p.ncells) = wnew;
-                if (has_aux && active) {
-                    const size_t gi = (size_t)((l * MM + q) * V + v) * p.ncells + cg;
-                    p.w_aux[gi] = fma(p.aux_c * p.scal[0], Ld, fma(p.aux_b, wp[l], p.aux_a * p.w_aux_in[gi]));
-                }
-                if (AV && p.do_sensor && v == 0) {
-                    sB = fma(wn[l], wn[l], sB);
-                    dB = fma(wn[l], Ld, dB);
-                    if (topxy || l == M - 1) {
-                        sA = fma(wn[l], wn[l], sA);
-                        dA = fma(wn[l], Ld, dA);
+                    for (int j = 1; j < M; ++j) acc = fma(c_tab.VtG[l * 8 + j], in[j], acc);
+                    if (v < Vc) acc += c_tab.Pend[0][l] * hfz[k][1] - c_tab.Pend[1][l] * hfz[k][0];
+                    const double Ld = pref * acc;
+                    double wnew = Ld;
+                    if (!p.rhs_only) wnew = fma(cdt, Ld, fma(p.rk_b, hwp[k][l], p.rk_a * hwn[k][l]));
+                    if (active) *row_ptr(bo, l * MM * V, p.ncells) = wnew;
+                    if (has_aux && active) {
+                        const size_t gi = (size_t)((l * MM + q) * V + v) * p.ncells + cg;
+                        p.w_aux[gi] = fma(p.aux_c * p.scal[0], Ld, fma(p.aux_b, hwp[k][l], p.aux_a * p.w_aux_in[gi]));
                     }
+                    if (AV && p.do_sensor && v == 0) {
+                        sB = fma(hwn[k][l], hwn[k][l], sB);
+                        dB = fma(hwn[k][l], Ld, dB);
+                        if (topxy || l == M - 1) {
+                            sA = fma(hwn[k][l], hwn[k][l], sA);
+                            dA = fma(hwn[k][l], Ld, dA);
+                        }
+                    }
+                    if (p.do_wavespeed) U[L::at2(v, q + l * MM) * C + cl] = wnew;
                 }
-                if (p.do_wavespeed) U[L::at2(v, q + l * MM) * C + cl] = wnew;
             }
         }
-    }
-    if (AV && p.do_sensor) {
-        // lanes of a warp that share a cell (lane = cl + C*j), then one partial per warp and cell in `sens`
-        constexpr int NW = NT / 32;
+        if (AV && p.do_sensor) {
+            // lanes of a warp that share a cell (lane = cl + C*j), then one partial per warp and cell in `sens`
+            constexpr int NW = NT / 32;
 #pragma unroll
-        for (int o = C; o < 32; o <<= 1) {
-            sA += __shfl_xor_sync(0xffffffffu, sA, o);
-            sB += __shfl_xor_sync(0xffffffffu, sB, o);
-            dA += __shfl_xor_sync(0xffffffffu, dA, o);
-            dB += __shfl_xor_sync(0xffffffffu, dB, o);
-        }
-        if ((tid & 31) < C) {
-            sens[(0 * NW + tid / 32) * C + cl] = sA;
-            sens[(1 * NW + tid / 32) * C + cl] = sB;
-            sens[(2 * NW + tid / 32) * C + cl] = dA;
-            sens[(3 * NW + tid / 32) * C + cl] = dB;
-        }
-        __syncthreads();
-        if (tid < C && cell0 + tid < p.ncells) {
-            double s[4] = {0.0, 0.0, 0.0, 0.0};
-            for (int k = 0; k < NW; ++k)
+            for (int o = C; o < 32; o <<= 1) {
+                sA += __shfl_xor_sync(0xffffffffu, sA, o);
+                sB += __shfl_xor_sync(0xffffffffu, sB, o);
+                dA += __shfl_xor_sync(0xffffffffu, dA, o);
+                dB += __shfl_xor_sync(0xffffffffu, dB, o);
+            }
+            if ((tid & 31) < C) {
+                sens[(0 * NW + tid / 32) * C + cl] = sA;
+                sens[(1 * NW + tid / 32) * C + cl] = sB;
+                sens[(2 * NW + tid / 32) * C + cl] = dA;
+                sens[(3 * NW + tid / 32) * C + cl] = dB;
+            }
+            __syncthreads();
+            if (tid < C && cell0 + tid < p.ncells) {
+                double s[4] = {0.0, 0.0, 0.0, 0.0};
+                for (int k = 0; k < NW; ++k)
 #pragma unroll
-                for (int i = 0; i < 4; ++i) s[i] += sens[(i * NW + k) * C + tid];
+                    for (int i = 0; i < 4; ++i) s[i] += sens[(i * NW + k) * C + tid];
+                const int c = cell0 + tid;
+                p.sens_new[c] = s[0] / s[1];
+                p.sens_new[p.ncells + c] = (s[0] > 0.0) ? (2.0 * s[2] / s[0] - 2.0 * s[3] / s[1]) : 0.0;
+            }
+        }
+        if (AV && p.commit_sensor && tid < C && cell0 + tid < p.ncells) {
             const int c = cell0 + tid;
-            p.sens_new[c] = s[0] / s[1];
-            p.sens_new[p.ncells + c] = (s[0] > 0.0) ? (2.0 * s[2] / s[0] - 2.0 * s[3] / s[1]) : 0.0;
+            p.sens_prev[c] = p.sens_new[c];
+            p.sens_prev[p.ncells + c] = p.sens_new[p.ncells + c];
         }
-    }
-    if (AV && p.commit_sensor && tid < C && cell0 + tid < p.ncells) {
-        const int c = cell0 + tid;
-        p.sens_prev[c] = p.sens_new[c];
-        p.sens_prev[p.ncells + c] = p.sens_new[p.ncells + c];
-    }
-    // ---- wave speeds of the new state for the next step's Eq. 23 ----
-    if (p.do_wavespeed) {
-        __syncthreads();
-        if (D == 3) expand_volume<D, M, C, NT, true, L>(U, Vc, tid);
-        wavespeed_points<D, M, C, NT, L>(U, p.gamma, p.flag, red, p.maxbits, tid);
+        // ---- wave speeds of the new state for the next step's Eq. 23 ----
+        if (p.do_wavespeed) {
+            __syncthreads();
+            if (D == 3) expand_volume<D, M, C, NT, true, L>(U, Vc, tid);
+            wavespeed_points<D, M, C, NT, L>(U, p.gamma, p.flag, red, p.maxbits, tid);
+        }
     }
 }
 

@@ -69,6 +69,18 @@ typedef struct dg_options {
 /* Fill *opt with the defaults above. */
 int dg_default_options(dg_options *opt);
 
+/* Run-time diagnostics of a solver (dg_get_diagnostics). */
+typedef struct dg_diagnostics {
+    double    t;               /* simulation time */
+    double    last_dt;         /* timestep of the last step (Eq. 23, or fixed_dt) */
+    double    c_max, v_max;    /* the two maxima of Eq. 23 that last_dt was computed from (reading A18) */
+    double    alpha_max_seen;  /* largest point value of alpha at a volume Gauss point over the states at the start of
+                                * every step since dg_set_state (alpha should stay below ~1); 0 without AV */
+    long long steps;           /* full RK steps since dg_set_state */
+    int       unphysical;      /* device flag, 0 = clean; bits: 1 volume point, 2 face point, 4 wave-speed pass,
+                                * 8 limiter cell mean saw rho <= 0 or p <= 0 */
+} dg_diagnostics;
+
 /* Create a solver (PAPER.md:175-190 operator on `mesh`; gamma of Eq. 5; nu, chi of Eq. 37-39; nu = chi = 0
  * selects the Euler path).  Allocates all device state; the state is zero until dg_set_state.
  * opt may be NULL (defaults).  Errors: DG_EINVAL, DG_ENOMEM, DG_ECUDA. */
@@ -81,6 +93,11 @@ int dg_init(dg_solver **out, const dg_mesh *mesh, int order, double gamma, doubl
 int dg_workspace_bytes(const dg_mesh *mesh, int order, const dg_options *opt, size_t *bytes);
 int dg_init_workspace(dg_solver **out, const dg_mesh *mesh, int order, double gamma, double nu, double chi,
                       const dg_options *opt, void *device_workspace, size_t bytes);
+
+/* Change the run-time options of an existing solver (f_cfl, fixed_dt, the AV factors of Eq. 43-46, alpha_max,
+ * use_graph, limiter_enable).  rk_stages and av_enable fix the device buffers and must equal the values given to
+ * dg_init (DG_EINVAL otherwise).  Takes effect at the next dg_step. */
+int dg_set_options(dg_solver *s, const dg_options *opt);
 
 /* Run all later work of this solver on `cuda_stream` (a cudaStream_t passed as void*; NULL = default
  * stream).  The Python binding passes torch's current stream. */
@@ -125,6 +142,18 @@ int dg_apply_limiter(dg_solver *s);
 
 /* Simulation time and the last timestep used (host pointers, either may be NULL). */
 int dg_get_time(dg_solver *s, double *t, double *last_dt);
+
+/* Time, last timestep, the Eq.-23 wave-speed maxima, the running maximum of alpha, step count and the
+ * unphysical-state flag in one call (`d` is a HOST pointer).  Synchronises the solver's stream. */
+int dg_get_diagnostics(dg_solver *s, dg_diagnostics *d);
+
+/* Checkpoint / restart of the lagged shock sensor ("two scalar quantities per cell"; reading
+ * A15): sg[0..N) = S^K, sg[N..2N) = G^K = d ln S / dt of the previous step; count = 2*Ncells; HOST or DEVICE pointer.
+ * A run is resumed bit-identically by dg_set_state + dg_set_alpha + dg_set_sensor + dg_set_time with the values read
+ * from dg_get_state / dg_get_alpha / dg_get_sensor / dg_get_time (dg_set_state zeroes alpha, sensor and t). */
+int dg_get_sensor(dg_solver *s, double *sg, size_t count);
+int dg_set_sensor(dg_solver *s, const double *sg, size_t count);
+int dg_set_time(dg_solver *s, double t);
 
 /* Launch geometry of the stage kernel of this solver (for bench.py / DESIGN.md): cells per block, threads
  * per block, dynamic shared memory bytes per block, number of blocks.  Any pointer may be NULL. */

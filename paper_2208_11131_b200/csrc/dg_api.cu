@@ -124,6 +124,7 @@ struct dg_solver {
     bool speeds_valid;
     cudaGraphExec_t graph;
     long long launches;
+    long long steps;        // full RK steps since dg_set_state
     int kC, kNT, kSmem;
 };
 
@@ -146,7 +147,7 @@ size_t workspace_layout(dg_solver *s, char *base) {
     s->WD = (s->opt.rk_stages == 5) ? (double *)take(sb) : nullptr;
     s->flux = (double *)take((size_t)s->dim * s->Vc * (s->M / s->order) * s->ncells * sizeof(double));
     s->scal = (double *)take(16 * sizeof(double));
-    s->maxbits = (unsigned long long *)take(2 * sizeof(unsigned long long));
+    s->maxbits = (unsigned long long *)take(4 * sizeof(unsigned long long));
     s->flag = (int *)take(sizeof(int));
     if (s->av) {
         s->sens_prev = (double *)take(2 * (size_t)s->ncells * sizeof(double));
@@ -481,6 +482,8 @@ int dg_set_state(dg_solver *s, const double *w, size_t count) {
     }
     CU(cudaMemsetAsync(s->scal, 0, 16 * sizeof(double), s->stream));
     CU(cudaMemsetAsync(s->flag, 0, sizeof(int), s->stream));
+    CU(cudaMemsetAsync(s->maxbits, 0, 4 * sizeof(unsigned long long), s->stream));
+    s->steps = 0;
     rc = enqueue_wavespeed(s);
     if (rc) return rc;
     CU(cudaStreamSynchronize(s->stream));   // the caller's buffer may be pageable / reused
@@ -544,6 +547,7 @@ int dg_step_async(dg_solver *s, int nsteps) {
         }
     }
     s->launches += (long long)nsteps * per_step;
+    s->steps += nsteps;
     return DG_OK;
 }
 
@@ -685,6 +689,75 @@ int dg_get_time(dg_solver *s, double *t, double *last_dt) {
     CU(cudaStreamSynchronize(s->stream));
     if (last_dt) *last_dt = v[0];
     if (t) *t = v[1];
+    return DG_OK;
+}
+
+int dg_set_options(dg_solver *s, const dg_options *opt) {
+    if (!s || !opt) return fail(DG_EINVAL, "NULL argument");
+    if (opt->rk_stages != s->opt.rk_stages || (opt->av_enable != 0) != (s->opt.av_enable != 0))
+        return fail(DG_EINVAL, "rk_stages and av_enable fix the device buffers: create a new solver to change them");
+    dg_mesh m;
+    std::memset(&m, 0, sizeof(m));
+    m.dim = s->dim;
+    for (int a = 0; a < 3; ++a) {
+        m.ncell[a] = s->ncell[a];
+        m.periodic[a] = 1;
+    }
+    m.h = s->h;
+    int rc = validate(&m, s->order, s->gamma, s->nu, s->chi, opt);
+    if (rc) return rc;
+    CU(cudaStreamSynchronize(s->stream));
+    s->opt = *opt;
+    drop_graph(s);              // the captured step carries the old options
+    s->speeds_valid = false;    // limiter on/off changes where the wave speeds are taken
+    return DG_OK;
+}
+
+int dg_get_diagnostics(dg_solver *s, dg_diagnostics *d) {
+    if (!s || !d) return fail(DG_EINVAL, "NULL argument");
+    double v[4];
+    unsigned long long mb[4];
+    int f = 0;
+    CU(cudaMemcpyAsync(v, s->scal, 4 * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    CU(cudaMemcpyAsync(mb, s->maxbits, 4 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, s->stream));
+    CU(cudaMemcpyAsync(&f, s->flag, sizeof(int), cudaMemcpyDeviceToHost, s->stream));
+    CU(cudaStreamSynchronize(s->stream));
+    d->last_dt = v[0];
+    d->t = v[1];
+    d->c_max = v[2];
+    d->v_max = v[3];
+    double a;
+    std::memcpy(&a, &mb[2], sizeof(double));
+    d->alpha_max_seen = s->av ? a : 0.0;
+    d->steps = s->steps;
+    d->unphysical = f;
+    return DG_OK;
+}
+
+int dg_get_sensor(dg_solver *s, double *sg, size_t count) {
+    if (!s || !sg) return fail(DG_EINVAL, "NULL argument");
+    if (count != 2 * (size_t)s->ncells) return fail(DG_EINVAL, "count must be 2*Ncells");
+    if (!s->av) return zero_fill(s, sg, count);
+    CU(cudaMemcpyAsync(sg, s->sens_prev, count * sizeof(double), cudaMemcpyDefault, s->stream));
+    CU(cudaStreamSynchronize(s->stream));
+    return DG_OK;
+}
+
+int dg_set_sensor(dg_solver *s, const double *sg, size_t count) {
+    if (!s || !sg) return fail(DG_EINVAL, "NULL argument");
+    if (!s->av) return fail(DG_EINVAL, "artificial viscosity is not enabled");
+    if (count != 2 * (size_t)s->ncells) return fail(DG_EINVAL, "count must be 2*Ncells");
+    CU(cudaMemcpyAsync(s->sens_prev, sg, count * sizeof(double), cudaMemcpyDefault, s->stream));
+    CU(cudaMemcpyAsync(s->sens_new, sg, count * sizeof(double), cudaMemcpyDefault, s->stream));
+    CU(cudaStreamSynchronize(s->stream));
+    return DG_OK;
+}
+
+int dg_set_time(dg_solver *s, double t) {
+    if (!s) return fail(DG_EINVAL, "solver is NULL");
+    if (!std::isfinite(t)) return fail(DG_EINVAL, "t must be finite");
+    CU(cudaMemcpyAsync(s->scal + 1, &t, sizeof(double), cudaMemcpyHostToDevice, s->stream));
+    CU(cudaStreamSynchronize(s->stream));
     return DG_OK;
 }
 

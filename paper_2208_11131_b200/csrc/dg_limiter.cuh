@@ -73,7 +73,7 @@ __global__ void __launch_bounds__(256, 2) dg_limiter_kernel(double *w, int V, in
     for (int mode = g; mode < Np; mode += G) {
 #pragma unroll
         for (int v = 0; v < Vc; ++v) {
-            const double x = __ldg(w + (size_t)(mode * V + v) * ncells + cg);
+            const double x = w[(size_t)(mode * V + v) * ncells + cg]   /* rewritten below: no non-coherent load */;
             RA[(v * Np + mode) * C + cl] = x;
             NV[(v * Np + mode) * C + cl] = x;
         }

@@ -955,6 +955,7 @@ __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(co
     {
         // V3: point-wise fluxes G_a = f_a - F_NS,a - eps d_a u (Eq. 24; 315 Eq. 38), alpha source
         bool bad = false;
+        double amax = 0.0;                                     // max alpha at the Gauss points (diagnostics)
         const double decay = (double)M / (p.f_tau * p.h);      // 1/tau = (n+1) c_s / (f_tau h), Eq. 44
         for (int it = tid; it < Np * C; it += NT) {
             const int cell = it % C;
@@ -978,6 +979,7 @@ __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(co
             if (AV) {
                 const double al = RA[L::at2(Vc, j) * C + cell];
                 const double cs = fast_sqrt(p.gamma * q.p * q.ir);
+                if (cell0 + cell < p.ncells) amax = fmax(amax, al);
                 eps = fmin(fmax(al, 0.0), p.alpha_max) * cs * (p.h / (double)M);        // Eq. 46, A17
                 // Eq. 43-45: shock source + wiggle source - decay; stored pre-scaled by h/2 for the projection
                 const double src = p.f_v * fmax(0.0, -divv) + Wk[cell] - al * (cs * decay);
@@ -997,8 +999,19 @@ __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(co
             }
         }
         if (bad) atomicOr(p.flag, 1);
+        if (AV && p.do_sensor) {
+            // running maximum of alpha over the states at the start of every step (dg_get_diagnostics)
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) amax = fmax(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+            if ((tid & 31) == 0) red[tid >> 5] = amax;
+        }
     }
     __syncthreads();
+    if (AV && p.do_sensor && tid == 0) {
+        double a = red[0];
+        for (int i = 1; i < NT / 32; ++i) a = fmax(a, red[i]);
+        atomic_max_nonneg(&p.maxbits[2], a);
+    }
     // Stage-combine inputs u^n and u^(i-1) of this thread's rows: issued before the last projection sweep so that
     // their latency is covered by it (same ownership as load_own_modes: modes g, g+G, ... of every variable).
     constexpr int CG = NT / C;
@@ -1012,7 +1025,7 @@ __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(co
         _Pragma("unroll") for (int k = 0; k < CNK; ++k) _Pragma("unroll") for (int v = 0; v < V; ++v) {     \
             wn[k][v] = wp[k][v] = 0.0;                                                                      \
             if (tid / C + k * CG < Np) {                                                                    \
-                if (need_n) wn[k][v] = __ldg(row_ptr(bn, k * CG * V + v, p.ncells));                        \
+                if (need_n) wn[k][v] = *row_ptr(bn, k * CG * V + v, p.ncells);    /* may alias w_out */                        \
                 if (need_p) wp[k][v] = __ldg(row_ptr(bp, k * CG * V + v, p.ncells));                        \
             }                                                                                               \
         }                                                                                                   \

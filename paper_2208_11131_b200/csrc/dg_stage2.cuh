@@ -165,6 +165,7 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), 1) dg_stage2_kerne
         {
             // ---- E: point-wise fluxes G_a = f_a - F_NS,a - eps d_a u (Eq. 24; 315 Eq. 38), alpha source ----
             bool bad = false;
+            double amax = 0.0;                                     // max alpha at the Gauss points (diagnostics)
             const double decay = (double)M / (p.f_tau * p.h);      // 1/tau = (n+1) c_s / (f_tau h), Eq. 44
             for (int it = tid; it < Np * C; it += NT) {
                 const int j = it / C;
@@ -187,6 +188,7 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), 1) dg_stage2_kerne
                 if (AV) {
                     const double al = U[L::at2(Vc, j) * C + cl];
                     const double cs = fast_sqrt(p.gamma * q.p * q.ir);
+                    if (active) amax = fmax(amax, al);
                     eps = fmin(fmax(al, 0.0), p.alpha_max) * cs * (p.h / (double)M);        // Eq. 46, A17
                     // Eq. 43-45: shock source + wiggle source - decay; stored pre-scaled by h/2 for the projection
                     const double src = p.f_v * fmax(0.0, -divv) + Wk[cl] - al * (cs * decay);
@@ -206,6 +208,12 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), 1) dg_stage2_kerne
                 }
             }
             if (bad) atomicOr(p.flag, 1);
+            if (AV && p.do_sensor) {
+                // running maximum of alpha over the states at the start of every step (dg_get_diagnostics)
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) amax = fmax(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+                if ((tid & 31) == 0) red[tid >> 5] = amax;
+            }
         }
         // face fluxes of this thread's G items, requested before the barrier: x faces as nodal values (jy, jz), y faces
         // modal in x and nodal in z (Cfg::PP); own cell = upper face, lower neighbour's = lower face
@@ -230,6 +238,11 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), 1) dg_stage2_kerne
             }
         }
         __syncthreads();
+        if (AV && p.do_sensor && tid == 0) {
+            double a = red[0];
+            for (int i = 1; i < NT / 32; ++i) a = fmax(a, red[i]);
+            atomic_max_nonneg(&p.maxbits[2], a);
+        }
 
         double sA = 0.0, sB = 0.0, dA = 0.0, dB = 0.0;      // shock-sensor sums of Eq. 42 (readings A13/A15)
 

@@ -9,7 +9,8 @@ struct DgStageArgs {
     double *w_aux;          // SSPRK(5,4) stage 4 only: aux_a u^(2) + aux_b u^(i-1) + aux_c dt L(u^(i-1)); NULL otherwise
     double *flux;           // projected upper-face fluxes [axis][var][transverse mode][cell] (face kernel -> stage kernel)
     const double *scal;     // device scalars: [0] = dt
-    unsigned long long *maxbits;  // [0] = bits of max c_s, [1] = bits of max |v| (non-negative doubles)
+    unsigned long long *maxbits;  // [0] = bits of max c_s, [1] = bits of max |v| (non-negative doubles; reset every step),
+                                  // [2] = bits of the running max of alpha at the Gauss points (reset by dg_set_state)
     int *flag;              // set to 1 on rho <= 0 or p <= 0
     double *sens_prev;      // [0..N) S^K, [N..2N) G^K of the previous step (AV only)
     double *sens_new;       // same, written on stage 1, committed to sens_prev on the last stage

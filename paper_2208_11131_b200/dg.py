@@ -36,6 +36,11 @@ class dg_options(C.Structure):
                 ("fixed_dt", C.c_double), ("use_graph", C.c_int), ("limiter_enable", C.c_int)]
 
 
+class dg_diagnostics(C.Structure):
+    _fields_ = [("t", C.c_double), ("last_dt", C.c_double), ("c_max", C.c_double), ("v_max", C.c_double),
+                ("alpha_max_seen", C.c_double), ("steps", C.c_longlong), ("unphysical", C.c_int)]
+
+
 # every symbol include/dg.h declares: name -> (restype, argtypes)
 _P = C.c_void_p
 SYMBOLS = {
@@ -56,6 +61,11 @@ SYMBOLS = {
     "dg_conserved_totals": (C.c_int, [_P, C.POINTER(C.c_double * 5)]),
     "dg_eval_rhs": (C.c_int, [_P, _P, C.c_size_t, _P, C.c_size_t]),
     "dg_get_time": (C.c_int, [_P, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
+    "dg_set_options": (C.c_int, [_P, C.POINTER(dg_options)]),
+    "dg_get_diagnostics": (C.c_int, [_P, C.POINTER(dg_diagnostics)]),
+    "dg_get_sensor": (C.c_int, [_P, _P, C.c_size_t]),
+    "dg_set_sensor": (C.c_int, [_P, _P, C.c_size_t]),
+    "dg_set_time": (C.c_int, [_P, C.c_double]),
     "dg_kernel_info": (C.c_int, [_P, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int)]),
     "dg_profile_stage": (C.c_int, [_P, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
     "dg_apply_limiter": (C.c_int, [_P]),
@@ -207,6 +217,32 @@ class Solver:
         t, dt = C.c_double(), C.c_double()
         _check(self._lib.dg_get_time(self._h, C.byref(t), C.byref(dt)))
         return t.value, dt.value
+
+    def set_options(self, **kw):
+        for k, v in kw.items():
+            if not hasattr(self.opt, k):
+                raise TypeError("unknown option " + k)
+            setattr(self.opt, k, v)
+        _check(self._lib.dg_set_options(self._h, C.byref(self.opt)))
+
+    def diagnostics(self):
+        d = dg_diagnostics()
+        _check(self._lib.dg_get_diagnostics(self._h, C.byref(d)))
+        return {k: getattr(d, k) for k, _ in dg_diagnostics._fields_}
+
+    def get_sensor(self, out=None):
+        if out is None:
+            out = np.empty(2 * self.ncells)
+        p, n, _keep = _buf(out)
+        _check(self._lib.dg_get_sensor(self._h, p, n))
+        return out
+
+    def set_sensor(self, sg):
+        p, n, _keep = _buf(sg)
+        _check(self._lib.dg_set_sensor(self._h, p, n))
+
+    def set_time(self, t):
+        _check(self._lib.dg_set_time(self._h, float(t)))
 
     def kernel_info(self):
         c, nt, sm, nb = C.c_int(), C.c_int(), C.c_int(), C.c_int()

@@ -291,3 +291,51 @@ def initial_modes_slabbed(wl: Workload, seed=SEED, layers=8, out=None):
         part = initial_modes(wl, seed, zslab=(z0, z1)).reshape(M * Vc, (z1 - z0) * plane)
         full[:, z0 * plane:z1 * plane] = part
     return out
+
+
+def supersonic_modes(dim, ncell, degree, gamma, axis, sign, mach=2.5, seed=SEED, amp=0.01):
+    """Seeded smooth state whose mean flow is supersonic along +/- `axis` (Mach ~ `mach`), so that every face normal
+    to that axis takes the fully upwinded branch of the Riemann solver (S_L >= 0 for sign = +1, S_R <= 0 for
+    sign = -1).  Cell means from primitive variables rho = 1, P = 1, v = sign * mach * c_s along the axis and
+    0.2 c_s on the other axes, each perturbed by 3 % per cell (so the mean pressure stays positive); higher modes iid
+    normal scaled by amp / (1 + sum l_a)^2.  Holds no method arithmetic beyond the definition of e (Eq. 2-3)."""
+    rng = np.random.default_rng(seed)
+    m = degree + 1
+    M = m ** dim
+    Vc = dim + 2
+    ncells = int(np.prod(ncell[:dim]))
+    cs = np.sqrt(gamma)
+    v0 = np.full(dim, 0.2 * cs)
+    v0[axis] = sign * mach * cs
+    rho = 1.0 + 0.03 * rng.standard_normal(ncells)
+    vel = v0[:, None] * (1.0 + 0.03 * rng.standard_normal((dim, ncells)))
+    prs = 1.0 + 0.03 * rng.standard_normal(ncells)
+    w = np.zeros((M, Vc, ncells))
+    w[0, 0] = rho
+    w[0, 1:1 + dim] = rho * vel
+    w[0, 1 + dim] = prs / (gamma - 1.0) + 0.5 * rho * np.sum(vel * vel, axis=0)
+    for mode in range(1, M):
+        rem, deg = mode, 0
+        for _ in range(dim):
+            deg += rem % m
+            rem //= m
+        w[mode] = amp * rng.standard_normal((Vc, ncells)) / (1.0 + deg) ** 2
+    return w.ravel()
+
+
+def alpha_field(dim, ncell, degree, lo=-0.2, hi=1.5, seed=SEED):
+    """Seeded artificial-viscosity field whose cell means cover [lo, hi] evenly (in random order) (both ends of the clamp
+    0 <= alpha <= alpha_max of Eq. 46 act), small higher modes; layout [mode*Ncells + cell]."""
+    rng = np.random.default_rng(seed + 17)
+    m = degree + 1
+    M = m ** dim
+    ncells = int(np.prod(ncell[:dim]))
+    a = np.zeros((M, ncells))
+    a[0] = rng.permutation(np.linspace(lo, hi, ncells))      # both ends are present on any mesh
+    for mode in range(1, M):
+        rem, deg = mode, 0
+        for _ in range(dim):
+            deg += rem % m
+            rem //= m
+        a[mode] = 0.03 * rng.standard_normal(ncells) / (1.0 + deg) ** 2
+    return a.ravel()

@@ -71,6 +71,82 @@ def test_rhs_parity(d, ncell, n, phys):
         assert np.max(np.abs(Lal - La)) < 5e-12 * max(1.0, np.max(np.abs(La)))
 
 
+# Supersonic mean flow along +/- every axis: the fully upwinded HLLC branches (S_L >= 0: left flux, S_R <= 0: right
+# flux, oracle.hllc_flux) decide every face normal to that axis, for every physics variant.
+SUPERSONIC_CASES = [(2, (5, 4), 2, a, sg, ph) for a in (0, 1) for sg in (1, -1) for ph in ("euler", "ns_av")] + \
+                   [(3, (3, 3, 2), 3, a, sg, ph) for a in (0, 1, 2) for sg in (1, -1) for ph in ("euler", "ns_av")] + \
+                   [(3, (2, 2, 2), 5, 2, -1, "euler"), (2, (5, 4), 0, 0, 1, "euler")]
+
+
+@pytest.mark.parametrize("d,ncell,n,axis,sign,phys", SUPERSONIC_CASES)
+def test_rhs_parity_supersonic(d, ncell, n, axis, sign, phys):
+    wl = _wl(d, ncell, n, phys)
+    w0 = wk.supersonic_modes(d, ncell, n, wl.gamma, axis, sign, mach=2.5, seed=23)
+    o, g = make_oracle(wl), make_gpu(wl)
+    o.set_state(w0)
+    g.set_state(w0)
+    if wl.av:
+        al = wk.alpha_field(d, ncell, n, lo=0.0, hi=0.6, seed=23)
+        o.set_alpha(al)
+        g.set_alpha(al)
+    # the case is what it claims to be: every cell mean is supersonic along the axis with the requested sign
+    mean = w0.reshape(wl.modes, d + 2, -1)[0]
+    vel = mean[1 + axis] / mean[0]
+    pres = (wl.gamma - 1.0) * (mean[d + 1] - 0.5 * np.sum(mean[1:1 + d] ** 2, axis=0) / mean[0])
+    assert np.all(sign * vel > 1.5 * np.sqrt(wl.gamma * pres / mean[0]))
+    L = o.rhs(o.w)
+    Lg, Lal = g.eval_rhs(with_alpha=True)
+    Vc = d + 2
+    Lo = np.ascontiguousarray(L[:, :, :Vc].transpose(1, 2, 0)).ravel()
+    err = np.max(np.abs(Lg - Lo).reshape(wl.modes, Vc, -1), axis=(0, 2)) / rhs_scale(Lo, wl)
+    assert np.all(err < 5e-12), err
+    if wl.av:
+        La = np.ascontiguousarray(L[:, :, Vc].T).ravel()
+        assert np.max(np.abs(Lal - La)) < 5e-12 * max(1.0, np.max(np.abs(La)))
+
+
+@pytest.mark.parametrize("d,ncell,n,axis,sign", [(2, (6, 5), 3, 0, 1), (2, (6, 5), 3, 1, -1), (3, (4, 3, 3), 3, 2, 1),
+                                                 (3, (4, 3, 3), 3, 0, -1)])
+def test_step_parity_supersonic(d, ncell, n, axis, sign):
+    wl = _wl(d, ncell, n, "ns_av", f_cfl=0.2)
+    w0 = wk.supersonic_modes(d, ncell, n, wl.gamma, axis, sign, mach=2.0, seed=29)
+    o, g = make_oracle(wl), make_gpu(wl)
+    o.set_state(w0)
+    g.set_state(w0)
+    assert o.step(1) == 0
+    g.step(1)
+    e1 = parity_norm(g.get_state(), o.get_state(), wl)
+    assert np.all(e1 <= TOL_1), e1
+    assert o.step(4) == 0
+    g.step(4)
+    e5 = parity_norm(g.get_state(), o.get_state(), wl)
+    assert np.all(e5 <= TOL_10), e5
+    assert np.max(np.abs(g.get_alpha() - o.get_alpha())) <= TOL_10
+
+
+@pytest.mark.parametrize("d,ncell,n", [(2, (7, 3), 3), (2, (5, 3), 5), (3, (3, 3, 2), 3), (3, (2, 2, 2), 6)])
+def test_rhs_parity_alpha_clamp(d, ncell, n):
+    """alpha cell means spread over [-0.2, 1.5]: both ends of the clamp 0 <= alpha <= alpha_max = 1 of Eq. 46
+    (reading A17) act at volume and face points (A12)."""
+    wl = _wl(d, ncell, n, "ns_av")
+    w0, _ = wk.random_smooth_modes(d, ncell, n, wl.gamma, seed=31, amp=0.04)
+    al = wk.alpha_field(d, ncell, n, lo=-0.2, hi=1.5, seed=31)
+    assert np.min(al[:wl.ncells]) < -0.05 and np.max(al[:wl.ncells]) > 1.2
+    o, g = make_oracle(wl), make_gpu(wl)
+    o.set_state(w0)
+    g.set_state(w0)
+    o.set_alpha(al)
+    g.set_alpha(al)
+    L = o.rhs(o.w)
+    Lg, Lal = g.eval_rhs(with_alpha=True)
+    Vc = d + 2
+    Lo = np.ascontiguousarray(L[:, :, :Vc].transpose(1, 2, 0)).ravel()
+    err = np.max(np.abs(Lg - Lo).reshape(wl.modes, Vc, -1), axis=(0, 2)) / rhs_scale(Lo, wl)
+    assert np.all(err < 5e-12), err
+    La = np.ascontiguousarray(L[:, :, Vc].T).ravel()
+    assert np.max(np.abs(Lal - La)) < 5e-12 * max(1.0, np.max(np.abs(La)))
+
+
 # ---------------------------------------------------------------------------------------------------
 # step-level parity on the five BASELINE configs at oracle-sized meshes (same ICs, same options)
 # ---------------------------------------------------------------------------------------------------
@@ -218,6 +294,60 @@ def test_unphysical_state_is_reported():
     with pytest.raises(dg.DGError) as ei:
         g.step(1)
     assert ei.value.code == dg.DG_EUNPHYSICAL
+
+
+def test_set_options_and_diagnostics():
+    from paper_2208_11131_b200 import dg
+    wl = _scaled_config(3)                                  # Sod + AV
+    w0 = wk.initial_modes(wl)
+    o = make_oracle(wl)
+    g = make_gpu(wl)
+    o.set_state(w0)
+    g.set_state(w0)
+    assert o.step(3) == 0
+    g.step(3)
+    d = g.diagnostics()
+    assert d["steps"] == 3 and d["unphysical"] == 0
+    assert abs(d["t"] - o.t) <= 1e-14 * o.t and abs(d["last_dt"] - o.last_dt) <= 1e-14 * o.last_dt
+    assert d["c_max"] > 0.0 and d["v_max"] >= 0.0
+    # Eq. 23 from the reported maxima reproduces the reported timestep
+    assert abs(wl.f_cfl * wl.h / (2.0 * wl.order * (d["c_max"] + d["v_max"])) - d["last_dt"]) <= 1e-15
+    # running maximum of alpha at the Gauss points of the states at the start of steps 1..3 (oracle: nodal alpha)
+    assert 0.0 < d["alpha_max_seen"] < 1.0
+    # change a run-time option: the next steps follow the oracle run with the same change
+    o.opt.f_cfl = 0.1
+    g.set_options(f_cfl=0.1)
+    assert o.step(2) == 0
+    g.step(2)
+    assert np.all(parity_norm(g.get_state(), o.get_state(), wl) <= TOL_10)
+    assert abs(g.get_time()[1] - o.last_dt) <= 1e-14 * o.last_dt
+    with pytest.raises(dg.DGError) as ei:
+        g.set_options(rk_stages=5)
+    assert ei.value.code == dg.DG_EINVAL
+    g.opt.rk_stages = 3
+    with pytest.raises(dg.DGError):
+        g.set_options(f_tau=0.0)
+
+
+def test_checkpoint_restart_is_bitwise():
+    """A run split by a checkpoint (state, alpha, lagged sensor (S, G), time) continues bit-identically."""
+    wl = _scaled_config(3)                                  # Sod + AV: the sensor and the alpha ODE are active
+    w0 = wk.initial_modes(wl)
+    a = make_gpu(wl)
+    a.set_state(w0)
+    a.step(6)
+    ck = (a.get_state(), a.get_alpha(), a.get_sensor(), a.get_time()[0])
+    a.step(5)
+    ref = (a.get_state(), a.get_alpha(), a.get_sensor(), a.get_time())
+    b = make_gpu(wl)
+    b.set_state(ck[0])
+    b.set_alpha(ck[1])
+    b.set_sensor(ck[2])
+    b.set_time(ck[3])
+    b.step(5)
+    assert np.array_equal(b.get_state(), ref[0]) and np.array_equal(b.get_alpha(), ref[1])
+    assert np.array_equal(b.get_sensor(), ref[2]) and b.get_time() == ref[3]
+    assert np.max(np.abs(ck[2])) > 0.0                      # the checkpointed sensor was not trivially zero
 
 
 def test_bad_arguments():

@@ -453,3 +453,34 @@ def test_eq23_timestep_closed_form():
         w[:, 0, :] = np.array([rho, *(rho * v), p / 0.4 + 0.5 * rho * v @ v])
         dt = o.timestep(w)
         assert abs(dt - 0.3 * o.h / (2 * (n + 1) * (math.sqrt(1.4 * p / rho) + np.linalg.norm(v)))) < 1e-15
+
+
+def test_eq23_separate_maxima_in_different_cells():
+    """PAPER.md:204-206 (Eq. 23, reading A18): the two maxima are taken SEPARATELY over the mesh,
+    dt = f h / (2 (n+1) (max c_s + max |v|)).  One cell is fast and cold, another slow and hot, so the plausible
+    mistake max(c_s + |v|) gives a different (larger) timestep; piecewise-constant states make the point values equal
+    to the cell means, so both maxima are known in closed form."""
+    gamma = 1.4
+    for d, n in [(2, 0), (2, 2), (3, 1)]:
+        o = make(d, (3, 2, 2)[:d], n, gamma=gamma, f_cfl=0.4)
+        ncells = o.w.shape[0]
+        w = np.zeros_like(o.w)
+        # background: rho = 1, p = 1, at rest
+        w[:, 0, 0] = 1.0
+        w[:, 0, d + 1] = 1.0 / (gamma - 1.0)
+        # cell 0: fast and cold (|v| = 3, c_s = sqrt(1.4 * 0.1 / 2))
+        v0 = np.array([3.0, 0.0, 0.0][:d])
+        w[0, 0, 0] = 2.0
+        w[0, 0, 1:1 + d] = 2.0 * v0
+        w[0, 0, d + 1] = 0.1 / (gamma - 1.0) + 0.5 * 2.0 * v0 @ v0
+        # last cell: at rest and hot (c_s = sqrt(1.4 * 8 / 0.5))
+        w[ncells - 1, 0, 0] = 0.5
+        w[ncells - 1, 0, d + 1] = 8.0 / (gamma - 1.0)
+        cs_cold, cs_hot, cs_bg = math.sqrt(gamma * 0.1 / 2.0), math.sqrt(gamma * 8.0 / 0.5), math.sqrt(gamma)
+        cmax, vmax = o.wave_speeds(w)
+        assert abs(cmax - cs_hot) < 1e-14 and abs(vmax - 3.0) < 1e-14
+        dt = o.timestep(w)
+        right = 0.4 * o.h / (2 * (n + 1) * (cs_hot + 3.0))
+        wrong = 0.4 * o.h / (2 * (n + 1) * max(cs_cold + 3.0, cs_hot, cs_bg))
+        assert abs(dt - right) < 1e-15
+        assert abs(dt - wrong) > 0.2 * right

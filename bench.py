@@ -28,9 +28,10 @@ if ROOT not in sys.path:
 from paper_2208_11131_b200 import roofline as rl          # noqa: E402
 from paper_2208_11131_b200 import workloads as wk         # noqa: E402
 
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE dg_stage_kernel launch from the committed `ncu --set full`
-# capture (profiles/), keyed by (workload, degree); None where no capture exists.
-TRAFFIC_BYTES = {("cfg4", 3): 18.275670e9 + 6.422608e9}   # profiles/r1g_cfg4_final.md
+# dram__bytes_read.sum + dram__bytes_write.sum of one RK stage = one dg_face_kernel launch + one dg_stage2_kernel launch
+# (the middle RK3 stage, which reads u^n and u^(i-1)), from the newest committed ncu capture under profiles/, keyed by
+# (workload, degree).  A constant from that capture, not a live measurement; None where no capture exists.
+TRAFFIC_BYTES = {("cfg4", 3): {"face": 11.31e9, "stage": 23.7e9, "source": "profiles/r2_cfg4.md"}}
 
 METRIC = "DG DoF-updates/sec (fp64, per RK stage)"
 UNIT = "DoF-updates/s"
@@ -218,7 +219,8 @@ def run_gpu(args):
         if use_dist:
             dist.destroy_process_group()
         return
-    # ---- roofline: the dominant kernel (dg_stage_kernel) from its own live CUDA-event time, and the whole stage ----
+    # ---- roofline: the WHOLE stage (face + stage kernel) from the timed region against the roof
+    #      that binds it; the two kernels with their own implementation traffic as sub-entries ----
     hbm_gbs, which = measured_peaks()
     t_stage = t_dev / (3 * args.steps)                       # face + stage kernel (+ 1/3 dt kernel), timed region
     face_ms, stage_ms = solver.profile_stage(3)              # per-kernel device time, events around each launch
@@ -228,31 +230,40 @@ def run_gpu(args):
     fl_face = rl.face_kernel_flops_per_cell(wl.dim, wl.m, visc, wl.av) * wl.ncells
     fl_stage = rl.stage_kernel_flops_per_cell(wl.dim, wl.m, visc, wl.av) * wl.ncells
     by_face, by_stage = (b * wl.ncells for b in rl.kernel_bytes_per_cell(wl.dim, wl.m, wl.av))
-    # which roof binds the stage kernel: time at the fp64 peak vs time at the HBM peak
-    t_alu, t_hbm = fl_stage / (rl.NOMINAL_FP64_TFLOPS * 1e12), by_stage / (hbm_gbs * 1e9)
-    if t_alu >= t_hbm:
-        roof = {"bound": "alu", "achieved": fl_stage / (stage_ms * 1e-3) / 1e12, "peak": rl.NOMINAL_FP64_TFLOPS,
-                "unit": "TFLOP/s", "peak_source": "nominal 148 SM x 64 DFMA/clk x 2 x 1.965 GHz (DESIGN.md section 6)"}
+    if r["bound"] == "alu":
+        roof = {"bound": "alu", "achieved": r["achieved_tflops"], "peak": rl.NOMINAL_FP64_TFLOPS, "unit": "TFLOP/s",
+                "frac": r["alu_frac"],
+                "peak_source": "148 SM x 64 DFMA/clk x 2 x 1.965 GHz (DESIGN.md section 6); measured DFMA loop beside it"}
     else:
-        roof = {"bound": "hbm", "achieved": by_stage / (stage_ms * 1e-3) / 1e9, "peak": hbm_gbs, "unit": "GB/s",
+        roof = {"bound": "hbm", "achieved": r["achieved_gbs"], "peak": hbm_gbs, "unit": "GB/s", "frac": r["hbm_frac"],
                 "peak_source": "%s HBM copy (MEASURED_PEAKS.json)" % which}
-    roof["frac"] = roof["achieved"] / roof["peak"]
+    tr = TRAFFIC_BYTES.get((args.workload, wl.degree))
     roof.update({
-        "traffic": TRAFFIC_BYTES.get((args.workload, wl.degree)), "kernel": "dg_stage_kernel",
-        "ms_per_launch": stage_ms, "alg_flops_per_launch": fl_stage, "alg_bytes_per_launch": by_stage,
-        "hbm_frac": by_stage / (stage_ms * 1e-3) / 1e9 / hbm_gbs,
-        "face_kernel": {"ms_per_launch": face_ms, "alg_flops_per_launch": fl_face, "alg_bytes_per_launch": by_face,
-                        "alu_frac": fl_face / (face_ms * 1e-3) / 1e12 / rl.NOMINAL_FP64_TFLOPS,
-                        "hbm_frac": by_face / (face_ms * 1e-3) / 1e9 / hbm_gbs},
-        "whole_stage": {"ms": t_stage * 1e3, "alg_flops_per_cell": r["flops_per_launch"] / wl.ncells,
-                        "alg_bytes_per_cell": r["bytes_per_launch"] / wl.ncells, "alu_frac": r["alu_frac"],
-                        "hbm_frac": r["hbm_frac"], "alg_tflops": r["achieved_tflops"], "alg_gbs": r["achieved_gbs"]},
-        "fp64_peak_measured_tflops": fp64_meas, "hbm_peak_gbs": hbm_gbs,
-        "note": "per-kernel times from dg_profile_stage (dw/dt evaluation path); whole_stage from the timed region"})
+        "traffic": (tr["face"] + tr["stage"]) if tr else None,
+        "traffic_source": (tr["source"] + " (committed capture, not live)") if tr else None,
+        "scope": "whole RK stage = dg_face_kernel + dg_stage kernel, timed region / (3 * steps)",
+        "ms_per_stage": t_stage * 1e3, "alg_flops_per_stage": r["flops_per_launch"],
+        "alg_bytes_per_stage": r["bytes_per_launch"], "alu_frac": r["alu_frac"], "hbm_frac": r["hbm_frac"],
+        "alg_flops_per_cell": r["flops_per_launch"] / wl.ncells, "alg_bytes_per_cell": r["bytes_per_launch"] / wl.ncells,
+        "kernels": {
+            "face": {"ms_per_launch": face_ms, "alg_flops_per_launch": fl_face,
+                     "implementation_bytes_per_launch": by_face, "dram_traffic_capture": tr["face"] if tr else None,
+                     "alu_frac": fl_face / (face_ms * 1e-3) / 1e12 / rl.NOMINAL_FP64_TFLOPS,
+                     "hbm_frac_of_implementation_bytes": by_face / (face_ms * 1e-3) / 1e9 / hbm_gbs},
+            "stage": {"ms_per_launch": stage_ms, "alg_flops_per_launch": fl_stage,
+                      "implementation_bytes_per_launch": by_stage, "dram_traffic_capture": tr["stage"] if tr else None,
+                      "alu_frac": fl_stage / (stage_ms * 1e-3) / 1e12 / rl.NOMINAL_FP64_TFLOPS,
+                      "hbm_frac_of_implementation_bytes": by_stage / (stage_ms * 1e-3) / 1e9 / hbm_gbs},
+            "note": "per-kernel times: dg_profile_stage, the middle RK3 stage with its real combine arguments; "
+                    "implementation bytes = what the two-kernel design must move (state read twice, flux buffer), "
+                    "not the algorithmic bytes of the headline"},
+        "fp64_peak_measured_tflops": fp64_meas, "hbm_peak_gbs": hbm_gbs})
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         v, cores, text, wall = oracle_sample(wl)
-        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": text, "seconds": wall}
+        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": text, "seconds": wall,
+               "host_cores": os.cpu_count(), "note": "the numpy oracle is single-threaded: %d of %d host cores" % (
+                   cores, os.cpu_count() or 0)}
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": t_max / args.steps * 1e3, "higher_is_better": True,
@@ -275,25 +286,40 @@ def run_gpu(args):
 
 
 def run_reference(args):
-    """Reference arm = the CPU oracle as it stands (this tier has no reference implementation), rank 0 only."""
+    """Reference arm = the CPU oracle as it stands (this tier has no reference implementation), rank 0 only:
+    W warm-up + exactly K timed RK3 steps of the oracle on a bounded sample of the workload (same ICs, physics and
+    degree on a coarser mesh of the same domain, sized so that one step takes a second or two)."""
     rank, world, _ = dist_env()
     if rank != 0:
         return
+    from oracle import dg_oracle as orc
     wl, label = pick_workload(args.workload, args.degree)
-    vals, walls, cores, text = [], [], 1, ""
-    for _ in range(max(1, min(args.steps, 3))):
-        v, cores, text, wall = oracle_sample(wl)
-        vals.append(v)
-        walls.append(wall)
-    v = float(np.median(vals))
+    per_cell = wl.modes ** 2 * wl.nvar
+    budget_cells = max(8, int(1.5e7 / per_cell))
+    n1 = min(max(2, int(round(budget_cells ** (1.0 / wl.dim)))), wl.ncell[0])
+    ncell = tuple(max(2, int(round(n1 * wl.ncell[a] / wl.ncell[0]))) for a in range(wl.dim))
+    sub = wk.with_mesh(wl, ncell)
+    o = orc.DGOracle(sub.dim, sub.ncell, sub.h, sub.order, sub.gamma, sub.nu, sub.chi,
+                     orc.Options(f_cfl=sub.f_cfl, av_enable=sub.av))
+    o.set_state(wk.initial_modes(sub))
+    o.step(args.warmup)
+    c0, t0 = time.process_time(), time.perf_counter()
+    o.step(args.steps)
+    wall = time.perf_counter() - t0
+    cores = max(1, int(round((time.process_time() - c0) / wall)))
+    v = sub.ncells * sub.modes * sub.nvar * 3 * args.steps / wall
+    text = "%d RK3 steps of the numpy oracle on %s cells (same ICs/physics/degree as the workload)" % (
+        args.steps, "x".join(str(c) for c in sub.ncell))
     line = {
         "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": float(np.median(walls)) / 2 * 1e3, "higher_is_better": True,
+        "warmup": args.warmup, "ms_per_step": wall / args.steps * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": label, "cells": wl.ncells, "modes_per_cell": wl.modes, "variables": wl.nvar,
-                   "rk_stages": 3, "note": "each step is a bounded sample of the workload (coarser mesh, same "
-                                           "ICs/physics/degree); ms_per_step is per sample RK3 step"},
-        "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": text},
+                   "rk_stages": 3, "sample_cells": sub.ncells,
+                   "note": "each timed step is one RK3 step on the bounded sample mesh (%s cells), not on the full "
+                           "workload; value = sample DoF-updates / wall time" % "x".join(str(c) for c in sub.ncell)},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": text,
+                         "host_cores": os.cpu_count()},
         "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }

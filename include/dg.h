@@ -64,6 +64,10 @@ typedef struct dg_options {
     double fixed_dt;     /* > 0: use this dt instead of Eq. 23; default 0 */
     int    use_graph;    /* 1: replay each time step as a CUDA graph (default); 0: plain launches */
     int    limiter_enable; /* 1: positivity limiter (Eq. 47) on the output of every RK stage; default 0 */
+    int    basis;        /* 0 (default): all (n+1)^dim tensor products (BASELINE.json mode counts); 1: the paper's
+                          * total-degree set, products with l_x+l_y(+l_z) > n are discarded (Eq. 17-18):
+                          * same storage layout, the discarded rows are zeroed by dg_set_state / dg_set_alpha and stay
+                          * zero; the sensor of Eq. 42 then uses the modes with l_x+l_y(+l_z) = n */
 } dg_options;
 
 /* Fill *opt with the defaults above. */

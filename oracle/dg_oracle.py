@@ -7,7 +7,8 @@ generator or helper with the CUDA path under `paper_2208_11131_b200/csrc/`; neit
 It is the plain, slow, literal algorithm: dense per-cell basis matrices (no sum factorisation), numpy fp64,
 Legendre values by three-term recurrence, every step in the paper's order and notation:
 
-  O1  basis            PAPER.md:121-139 (Eq. 13-16), tensor-product mode set (reading A1)
+  O1  basis            PAPER.md:121-139 (Eq. 13-16), tensor-product mode set (reading A1); option
+                       basis="total_degree": the paper's truncated set, PAPER.md:141-148 (Eq. 17-18)
   O2  quadrature       PAPER.md:164-171 (Eq. 19), n_g = n+1
   O3  timestep         PAPER.md:202-206 (Eq. 23), p = n+1 (A2)
   O4  RHS (weak form)  PAPER.md:104 (Eq. 10), 175-190 (Eq. 20-21); prefactors per A3/A4
@@ -252,6 +253,9 @@ class Options:
     alpha_max: float = 1.0
     fixed_dt: float = 0.0  # > 0: use this dt instead of Eq. 23
     limiter_enable: bool = False  # positivity limiter after every RK stage (Eq. 47)
+    # mode set: "tensor" = all (n+1)^d products (reading A1, BASELINE.json mode counts); "total_degree" = the paper's
+    # own set, products whose total degree sum_a l_a exceeds n are discarded (Eq. 17-18)
+    basis: str = "tensor"
 
 
 class DGOracle:
@@ -330,6 +334,19 @@ class DGOracle:
                 rem //= m
             lmax[idx] = mx
         self.top = (lmax == n) if n >= 1 else np.zeros(self.M, dtype=bool)
+        # total-degree truncation: keep[l] = (sum_a l_a <= n).  The basis is orthonormal, so the
+        # Galerkin equations of the kept modes are those of Eq. 20 unchanged and the discarded weights stay zero;
+        # the "highest-order" modes of the sensor (Eq. 42: l = N_{p-1}+1 .. N_p) are then those with sum_a l_a = n.
+        assert self.opt.basis in ("tensor", "total_degree")
+        lsum = np.zeros(self.M, dtype=int)
+        for idx in range(self.M):
+            rem = idx
+            for _ in range(d):
+                lsum[idx] += rem % m
+                rem //= m
+        self.keep = (lsum <= n) if self.opt.basis == "total_degree" else np.ones(self.M, dtype=bool)
+        if self.opt.basis == "total_degree":
+            self.top = (lsum == n) if n >= 1 else np.zeros(self.M, dtype=bool)
 
     def _build_neighbours(self):
         d = self.d
@@ -347,6 +364,7 @@ class DGOracle:
         assert w_flat.size == self.M * self.Vc * self.ncells
         self.w[:] = 0.0
         self.w[:, :, :self.Vc] = w_flat.reshape(self.M, self.Vc, self.ncells).transpose(2, 0, 1)
+        self.w[:, ~self.keep, :] = 0.0          # L2 projection onto the kept (orthonormal) modes
         self.sensor_S[:] = 0.0
         self.sensor_G[:] = 0.0
         self.t = 0.0
@@ -365,6 +383,7 @@ class DGOracle:
     def set_alpha(self, a_flat):
         assert self.av
         self.w[:, :, self.Vc] = np.asarray(a_flat, dtype=np.float64).reshape(self.M, self.ncells).T
+        self.w[:, ~self.keep, self.Vc] = 0.0
 
     def conserved_totals(self):
         """|K| sum_cells w_0 per conserved variable (O12), compensated summation."""
@@ -464,6 +483,9 @@ class DGOracle:
             sur[:, :, :Vc] -= pref * np.einsum("k,ckv,kl->clv", self.gsur, Fh, self.PhiF[a][1])
             contrib = pref * np.einsum("k,ckv,kl->clv", self.gsur, Fh, self.PhiF[a][0])
             sur[R, :, :Vc] += contrib          # R is a permutation of the cells: no duplicate indices
+        # total-degree basis: only the kept modes are test functions of Eq. 20
+        vol[:, ~self.keep, :] = 0.0
+        sur[:, ~self.keep, :] = 0.0
         if terms:
             return vol + sur, vol, sur
         return vol + sur

@@ -90,6 +90,22 @@ __global__ void __launch_bounds__(1024) dg_totals_kernel(const double *w, int V,
     if (threadIdx.x == 0) out[v] = vol * (ss[0] + sc[0]);
 }
 
+// total-degree basis: zero the rows of the discarded modes (sum_a l_a > n) of `nv` variables
+__global__ void dg_mask_modes_kernel(double *w, int pitch_vars, int var0, int nv, int nmodes, int m, int dim, int ncells) {
+    const size_t total = (size_t)nmodes * nv * ncells;
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+        const int cell = (int)(i % ncells);
+        const int r = (int)(i / ncells);
+        const int mode = r / nv, v = r % nv;
+        int rem = mode, lsum = 0;
+        for (int a = 0; a < dim; ++a) {
+            lsum += rem % m;
+            rem /= m;
+        }
+        if (lsum > m - 1) w[((size_t)mode * pitch_vars + var0 + v) * ncells + cell] = 0.0;
+    }
+}
+
 // register-resident DFMA loop: 8 independent chains per thread
 __global__ void __launch_bounds__(256) dg_dfma_kernel(double *out, int iters, double a, double b) {
     double x0 = threadIdx.x, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
@@ -175,6 +191,7 @@ int validate(const dg_mesh *mesh, int order, double gamma, double nu, double chi
     if (o->rk_stages != 1 && o->rk_stages != 2 && o->rk_stages != 3 && o->rk_stages != 5)
         return fail(DG_EINVAL, "rk_stages must be 1, 2, 3 or 5");
     if (!(o->f_cfl > 0.0) && !(o->fixed_dt > 0.0)) return fail(DG_EINVAL, "f_cfl must be positive");
+    if (o->basis != 0 && o->basis != 1) return fail(DG_EINVAL, "basis must be 0 (tensor product) or 1 (total degree)");
     if (o->av_enable) {
         if (!(o->f_tau > 0.0)) return fail(DG_EINVAL, "f_tau must be positive (Eq. 44 divides by it)");
         if (!(o->f_v >= 0.0) || !(o->f_w >= 0.0)) return fail(DG_EINVAL, "f_v and f_w must be non-negative");
@@ -205,6 +222,7 @@ void fill_args(const dg_solver *s, DgStageArgs *a) {
     a->f_w = s->opt.f_w;
     a->s_onset = s->opt.s_onset0 / ((double)s->order * (double)s->order);
     a->alpha_max = s->opt.alpha_max;
+    a->total_degree = s->opt.basis ? 1 : 0;
 }
 
 // enqueue the wave-speed evaluation of the current state (Eq. 23 inputs for the next step)
@@ -440,6 +458,7 @@ int dg_default_options(dg_options *opt) {
     opt->fixed_dt = 0.0;
     opt->use_graph = 1;
     opt->limiter_enable = 0;
+    opt->basis = 0;
     return DG_OK;
 }
 
@@ -476,6 +495,10 @@ int dg_set_state(dg_solver *s, const double *w, size_t count) {
     CU(cudaMemsetAsync(s->W0, 0, s->nstate * sizeof(double), s->stream));
     int rc = copy_vars(s, s->W0, s->V, w, s->Vc, s->Vc);
     if (rc) return rc;
+    if (s->opt.basis) {     // L2 projection onto the kept (orthonormal) modes
+        dg_mask_modes_kernel<<<1024, 256, 0, s->stream>>>(s->W0, s->V, 0, s->Vc, s->M, s->order, s->dim, s->ncells);
+        CU(cudaGetLastError());
+    }
     if (s->av) {
         CU(cudaMemsetAsync(s->sens_prev, 0, 2 * (size_t)s->ncells * sizeof(double), s->stream));
         CU(cudaMemsetAsync(s->sens_new, 0, 2 * (size_t)s->ncells * sizeof(double), s->stream));
@@ -496,6 +519,10 @@ int dg_set_alpha(dg_solver *s, const double *alpha, size_t count) {
     if (count != (size_t)s->M * s->ncells) return fail(DG_EINVAL, "count must be M*Ncells");
     int rc = copy_vars(s, s->W0 + (size_t)s->Vc * s->ncells, s->V, alpha, 1, 1);
     if (rc) return rc;
+    if (s->opt.basis) {
+        dg_mask_modes_kernel<<<1024, 256, 0, s->stream>>>(s->W0, s->V, s->Vc, 1, s->M, s->order, s->dim, s->ncells);
+        CU(cudaGetLastError());
+    }
     CU(cudaStreamSynchronize(s->stream));
     return DG_OK;
 }
@@ -696,6 +723,7 @@ int dg_set_options(dg_solver *s, const dg_options *opt) {
     if (!s || !opt) return fail(DG_EINVAL, "NULL argument");
     if (opt->rk_stages != s->opt.rk_stages || (opt->av_enable != 0) != (s->opt.av_enable != 0))
         return fail(DG_EINVAL, "rk_stages and av_enable fix the device buffers: create a new solver to change them");
+    if (opt->basis != s->opt.basis) return fail(DG_EINVAL, "the mode set (basis) cannot change under a loaded state");
     dg_mesh m;
     std::memset(&m, 0, sizeof(m));
     m.dim = s->dim;

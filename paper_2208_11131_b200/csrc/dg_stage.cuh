@@ -1117,16 +1117,21 @@ __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(co
 #pragma unroll
         for (int k = 0; k < NK; ++k) {
             const int mode = g + k * G;
-            int rem = mode, top = 0;
+            int rem = mode, top = 0, lsum = 0;
 #pragma unroll
             for (int a = 0; a < D; ++a) {
                 top |= (rem % M == M - 1);
+                lsum += rem % M;
                 rem /= M;
             }
+            // total-degree basis: discarded modes are not test functions; the sensor's highest
+            // modes are those with sum_a l_a = n
+            const bool keep = !p.total_degree || (lsum <= M - 1);
+            if (p.total_degree) top = (lsum == M - 1);
 #pragma unroll
             for (int v = 0; v < V; ++v) {
                 if (mode < Np) {
-                    const double Ld = ACC[L::at2(v, mode) * C + cl];
+                    const double Ld = keep ? ACC[L::at2(v, mode) * C + cl] : 0.0;
                     double wnew = Ld;
                     if (!p.rhs_only) wnew = fma(cdt, Ld, fma(p.rk_b, wp[k][v], p.rk_a * wn[k][v]));
                     if (active) *row_ptr(bo, k * G * V + v, p.ncells) = wnew;

@@ -302,7 +302,8 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), 1) dg_stage2_kerne
                 }
 #pragma unroll
                 for (int q = 0; q < MM; ++q) {
-                    const double Ld = pref * n[q];
+                    const bool keep = !p.total_degree || (q % M + q / M <= M - 1);
+                    const double Ld = keep ? pref * n[q] : 0.0;
                     double wnew = Ld;
                     if (!p.rhs_only) wnew = fma(cdt, Ld, fma(p.rk_b, wp[q], p.rk_a * wn[q]));
                     if (active) *row_ptr(bo, q * V, p.ncells) = wnew;
@@ -311,7 +312,7 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), 1) dg_stage2_kerne
                         p.w_aux[gi] = fma(p.aux_c * p.scal[0], Ld, fma(p.aux_b, wp[q], p.aux_a * p.w_aux_in[gi]));
                     }
                     if (AV && p.do_sensor && v == 0) {
-                        const bool top = (q % M == M - 1) || (q / M == M - 1);
+                        const bool top = p.total_degree ? (q % M + q / M == M - 1) : ((q % M == M - 1) || (q / M == M - 1));
                         sB = fma(wn[q], wn[q], sB);
                         dB = fma(wn[q], Ld, dB);
                         if (top) {
@@ -367,13 +368,16 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), 1) dg_stage2_kerne
 #pragma unroll
                 for (int j = 0; j < M; ++j) in[j] = U[L::at2(v, q + j * MM) * C + cl];
                 const bool topxy = (q % M == M - 1) || (q / M == M - 1);
+                const int lxy = q % M + q / M;
 #pragma unroll
                 for (int l = 0; l < M; ++l) {
                     double acc = c_tab.VtG[l * 8] * in[0];
 #pragma unroll
                     for (int j = 1; j < M; ++j) acc = fma(c_tab.VtG[l * 8 + j], in[j], acc);
                     if (v < Vc) acc += c_tab.Pend[0][l] * hfz[k][1] - c_tab.Pend[1][l] * hfz[k][0];
-                    const double Ld = pref * acc;
+                    // total-degree basis: the discarded modes are not test functions of Eq. 20
+                    const bool keep = !p.total_degree || (lxy + l <= M - 1);
+                    const double Ld = keep ? pref * acc : 0.0;
                     double wnew = Ld;
                     if (!p.rhs_only) wnew = fma(cdt, Ld, fma(p.rk_b, hwp[k][l], p.rk_a * hwn[k][l]));
                     if (active) *row_ptr(bo, l * MM * V, p.ncells) = wnew;
@@ -384,7 +388,7 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), 1) dg_stage2_kerne
                     if (AV && p.do_sensor && v == 0) {
                         sB = fma(hwn[k][l], hwn[k][l], sB);
                         dB = fma(hwn[k][l], Ld, dB);
-                        if (topxy || l == M - 1) {
+                        if (p.total_degree ? (lxy + l == M - 1) : (topxy || l == M - 1)) {
                             sA = fma(hwn[k][l], hwn[k][l], sA);
                             dA = fma(hwn[k][l], Ld, dA);
                         }

@@ -33,7 +33,7 @@ class dg_mesh(C.Structure):
 class dg_options(C.Structure):
     _fields_ = [("f_cfl", C.c_double), ("rk_stages", C.c_int), ("av_enable", C.c_int), ("f_v", C.c_double),
                 ("f_tau", C.c_double), ("f_w", C.c_double), ("s_onset0", C.c_double), ("alpha_max", C.c_double),
-                ("fixed_dt", C.c_double), ("use_graph", C.c_int), ("limiter_enable", C.c_int)]
+                ("fixed_dt", C.c_double), ("use_graph", C.c_int), ("limiter_enable", C.c_int), ("basis", C.c_int)]
 
 
 class dg_diagnostics(C.Structure):

@@ -134,6 +134,26 @@ def _sod(wl, X):
     return _conserved(rho, [zero] * wl.dim, P, wl.gamma)
 
 
+def vortex_exact(wl: Workload, X):
+    """Isentropic vortex of Yee et al. (Eq. 48-51) on [-5,5]^2, gamma = 1.4, beta = 5: a steady
+    solution of the Euler equations (the exact solution at any time is the initial state).  u = P/((gamma-1) rho) is
+    the thermal energy per unit mass, so P = (gamma-1) rho u = rho^gamma (isentropic)."""
+    x, y = X
+    beta = wl.params.get("beta", 5.0)
+    g = wl.gamma
+    r2 = x * x + y * y
+    f = (beta / (2.0 * np.pi)) * np.exp(0.5 * (1.0 - r2))
+    u = 1.0 - (beta * beta / (8.0 * g * np.pi ** 2)) * np.exp(1.0 - r2)
+    rho = ((g - 1.0) * u) ** (1.0 / (g - 1.0))
+    return _conserved(rho, [-y * f, x * f], (g - 1.0) * rho * u, g)
+
+
+def vortex(ncell=32, degree=3) -> Workload:
+    """The isentropic-vortex workload: 2D Euler, periodic box [-5,5]^2."""
+    return Workload("vortex2d", 2, (ncell, ncell), 10.0 / ncell, degree, 1.4, f_cfl=0.3, steps=10, ic="vortex",
+                    origin=(-5.0, -5.0, 0.0), params=dict(beta=5.0))
+
+
 def turbulence_modes(wl: Workload, seed=SEED):
     """Half-space integer wave vectors with kmin <= |k| <= kmax and their solenoidal complex amplitudes
     a_k -> (I - k k^T/k^2) a_k, a_k iid complex standard normal (flat spectrum), SURVEY.md 8(d) item 4."""
@@ -226,6 +246,8 @@ def initial_modes(wl: Workload, seed=SEED, zslab=None):
             U = _kh(wl, grids)
         elif wl.ic == "sod":
             U = _sod(wl, grids)
+        elif wl.ic == "vortex":
+            U = vortex_exact(wl, grids)
         elif wl.ic == "uniform":
             one = np.ones_like(grids[0])
             U = _conserved(one, [0.0 * one] * d, one, wl.gamma)

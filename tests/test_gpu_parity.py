@@ -525,3 +525,56 @@ def test_limiter_steps_parity_and_inactive_bitwise():
     tg, dtg = g.get_time()
     assert abs(dtg - o.last_dt) <= 1e-12 * o.last_dt
     _report("limiter inside RK3, 2D degree 2 AV, 2 steps from a limited rough state: %.3e" % np.max(e))
+
+
+# ---------------------------------------------------------------------------------------------------
+# total-degree-truncated basis (Eq. 17-18) and the isentropic vortex
+# (Eq. 48-51)
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("d,ncell,n,phys", [(2, (5, 3), 3, "ns_av"), (2, (6, 4), 5, "av"), (3, (3, 2, 2), 3, "ns_av"),
+                                            (3, (2, 2, 2), 2, "euler"), (3, (2, 2, 2), 6, "euler")])
+def test_total_degree_basis_parity(d, ncell, n, phys):
+    wl = _wl(d, ncell, n, phys, f_cfl=0.2)
+    w0, al = wk.random_smooth_modes(d, ncell, n, wl.gamma, seed=41, amp=0.04, nvar_extra=1 if wl.av else 0)
+    o = make_oracle(wl, basis="total_degree")
+    g = make_gpu(wl, basis=1)
+    o.set_state(w0)
+    g.set_state(w0)
+    if wl.av:
+        o.set_alpha(al)
+        g.set_alpha(al)
+    assert np.array_equal(g.get_state(), o.get_state())          # the projection onto the kept modes is exact
+    keep = o.keep
+    assert keep.sum() == ((n + 1) * (n + 2) * (n + 3) // 6 if d == 3 else (n + 1) * (n + 2) // 2)
+    assert o.step(1) == 0
+    g.step(1)
+    e1 = parity_norm(g.get_state(), o.get_state(), wl)
+    assert np.all(e1 <= TOL_1), e1
+    assert o.step(4) == 0
+    g.step(4)
+    wg = g.get_state()
+    assert np.all(parity_norm(wg, o.get_state(), wl) <= TOL_10)
+    assert np.max(np.abs(wg.reshape(wl.modes, d + 2, -1)[~keep])) == 0.0      # discarded rows stay exactly zero
+    if wl.av:
+        ag = g.get_alpha()
+        assert np.max(np.abs(ag - o.get_alpha())) <= TOL_10
+        assert np.max(np.abs(ag.reshape(wl.modes, -1)[~keep])) == 0.0
+
+
+def test_isentropic_vortex_parity_and_steadiness():
+    wl = wk.vortex(24, degree=3)
+    w0 = wk.initial_modes(wl)
+    o, g = make_oracle(wl), make_gpu(wl)
+    o.set_state(w0)
+    g.set_state(w0)
+    assert o.step(1) == 0
+    g.step(1)
+    assert np.all(parity_norm(g.get_state(), o.get_state(), wl) <= TOL_1)
+    assert o.step(9) == 0
+    g.step(9)
+    w10 = g.get_state()
+    assert np.all(parity_norm(w10, o.get_state(), wl) <= TOL_10)
+    # steady exact solution: after 10 steps the cell means moved by no more than the truncation error
+    d0 = w0.reshape(wl.modes, 4, -1)[0, 0]
+    d10 = w10.reshape(wl.modes, 4, -1)[0, 0]
+    assert np.mean(np.abs(d10 - d0)) < 1e-5

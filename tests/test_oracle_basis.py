@@ -156,3 +156,112 @@ def test_recovery_known_integrals_f1_n1():
     assert abs(Am[0, 0] - 1.0) < 1e-14 and abs(Am[0, 1] + math.sqrt(3) / 2) < 1e-14
     assert abs(Am[1, 0]) < 1e-14 and abs(Am[1, 1] - 0.5) < 1e-14
     assert abs(Ap[0, 1] - math.sqrt(3) / 2) < 1e-14
+
+
+# ---------------------------------------------------------------------------------------------------
+# total-degree-truncated basis (Eq. 17-18)
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("d", [2, 3])
+@pytest.mark.parametrize("n", [0, 1, 2, 3, 5, 7])
+def test_total_degree_mode_count_eq17_eq18(d, n):
+    """The kept set has N^3D(n) = (n+1)(n+2)(n+3)/6 (Eq. 17) / N^2D(n) = (n+1)(n+2)/2 (Eq. 18) members, every one
+    of total degree <= n, and the sensor's highest-order set (Eq. 42: l = N_{p-1}+1..N_p) has N(n) - N(n-1)."""
+    o = orc.DGOracle(d, (2,) * d, 0.5, n + 1, 1.4, options=orc.Options(basis="total_degree", av_enable=True))
+    N = (lambda k: (k + 1) * (k + 2) * (k + 3) // 6) if d == 3 else (lambda k: (k + 1) * (k + 2) // 2)
+    assert int(o.keep.sum()) == N(n)
+    for idx in np.nonzero(o.keep)[0]:
+        rem, s = int(idx), 0
+        for _ in range(d):
+            s += rem % (n + 1)
+            rem //= (n + 1)
+        assert s <= n
+    assert int(o.top.sum()) == (N(n) - N(n - 1) if n >= 1 else 0)
+    assert not np.any(o.top & ~o.keep)
+    # PAPER.md:771: "for p=2, N^3D is lower than p^3 by a factor 2", 3.2 at p=4 (ratios of the golden file)
+    if d == 3 and n in (1, 3):
+        assert abs((n + 1) ** 3 / o.keep.sum() - _gold("recovery_eq36.txt")["ratio_p%d" % (n + 1)]) < 1e-12
+
+
+@pytest.mark.parametrize("d,n", [(2, 2), (2, 3), (3, 2)])
+def test_total_degree_basis_represents_total_degree_polynomials_exactly(d, n):
+    """A polynomial of TOTAL degree <= n lies in the truncated space: projecting it (full tensor projection by
+    quadrature, then the mask of set_state) loses nothing, while x^n y^n (total degree 2n) does lose its high part."""
+    from numpy.polynomial import legendre as L
+    o = orc.DGOracle(d, (1,) * d, 2.0, n + 1, 1.4, options=orc.Options(basis="total_degree"))
+    xq, gq = L.leggauss(n + 3)
+    grids = np.meshgrid(*([xq] * d), indexing="ij")
+    pts = np.stack([g.ravel() for g in grids[::-1]], axis=1)
+    gw = np.ones(len(pts))
+    for a in range(d):
+        gw = gw * gq[np.searchsorted(xq, pts[:, a])]
+
+    def modes_of(f):
+        phi = o.evaluate(np.eye(o.M)[None, :, :].transpose(0, 2, 1) * 1.0, pts)[0]      # phi[j, l]
+        return (phi * (gw * f)[:, None]).sum(axis=0) / 2.0 ** d
+
+    x, y = pts[:, 0], pts[:, 1]
+    f_in = 0.3 + x ** n - 0.7 * x ** (n - 1) * y + (pts[:, 2] * y if d == 3 and n >= 2 else 0.0)
+    w = modes_of(f_in)
+    assert np.max(np.abs(w[~o.keep])) < 1e-13                    # nothing outside the kept set
+    f_out = x ** n * y ** n
+    assert np.max(np.abs(modes_of(f_out)[~o.keep])) > 1e-3
+
+
+def test_total_degree_rhs_is_the_tensor_rhs_on_the_kept_modes_and_conserves():
+    """Orthonormal basis: the Galerkin equations of the kept modes are Eq. 20 unchanged (a state that lives in the
+    truncated space gives the same dw/dt for the kept modes under both options, zero for the discarded ones);
+    mode 0 is kept, so conservation (Eq. 10 summed over cells) still holds to round-off."""
+    d, n = 2, 3
+    w0, _ = wk.random_smooth_modes(d, (4, 3), n, 1.4, seed=9, amp=0.05)
+    ot = orc.DGOracle(d, (4, 3), 0.25, n + 1, 1.4, 0.01, 0.02, orc.Options(basis="total_degree"))
+    of = orc.DGOracle(d, (4, 3), 0.25, n + 1, 1.4, 0.01, 0.02, orc.Options())
+    ot.set_state(w0)
+    of.set_state(ot.get_state())                                 # the truncated state, in the full space
+    Lt, Lf = ot.rhs(ot.w), of.rhs(of.w)
+    assert np.max(np.abs(Lt[:, ot.keep] - Lf[:, ot.keep])) == 0.0
+    assert np.max(np.abs(Lt[:, ~ot.keep])) == 0.0 and np.max(np.abs(Lf[:, ~ot.keep])) > 1e-6
+    assert np.max(np.abs(Lt[:, 0, :].sum(axis=0))) < 1e-12 * np.abs(Lt[:, 0, :]).sum()
+    assert ot.step(3) == 0
+    assert np.max(np.abs(ot.w[:, ~ot.keep])) == 0.0
+
+
+def test_total_degree_convergence_order():
+    """"the expected spatial convergence order due to the leading truncation error is in each case
+    p = n + 1" -- with the truncated set on the advected wave (BASELINE config 1), degree 2."""
+    import math
+    from test_oracle_physics import _l1_wave
+    n, errs = 2, []
+    for N in (8, 16):
+        wl = wk.with_mesh(wk.config(1, degree=n), (N, N))
+        o = orc.DGOracle(2, wl.ncell, wl.h, wl.order, wl.gamma, options=orc.Options(f_cfl=0.1, basis="total_degree"))
+        o.set_state(wk.initial_modes(wl))
+        while o.t < 0.05 - 1e-14:
+            o.opt.fixed_dt = 0.0
+            o.opt.fixed_dt = min(o.timestep(o.w), 0.05 - o.t)
+            o.step(1)
+        errs.append(_l1_wave(o, wl, o.t))
+    rate = math.log(errs[0] / errs[1]) / math.log(2.0)
+    assert rate > n + 1 - 0.4, (errs, rate)
+
+
+# ---------------------------------------------------------------------------------------------------
+# isentropic vortex (Eq. 48-51): a steady Euler solution
+# ---------------------------------------------------------------------------------------------------
+def test_isentropic_vortex_is_steady_and_converges():
+    """dw/dt of the projected vortex -> 0 under refinement at rate ~ h^n (the residual of a steady exact solution is
+    the truncation error), and the state is isentropic: P = rho^gamma at the projected cell centres."""
+    import math
+    res = []
+    for N in (8, 16):
+        wl = wk.vortex(N, degree=2)
+        o = orc.DGOracle(2, wl.ncell, wl.h, wl.order, wl.gamma)
+        o.set_state(wk.initial_modes(wl))
+        Lw = o.rhs(o.w)
+        res.append(np.sqrt(np.mean(Lw[:, :, 0] ** 2)))
+    assert res[1] < res[0] / 3.0, res
+    X = np.meshgrid(np.linspace(-2, 2, 5), np.linspace(-2, 2, 5))
+    rho, mx, my, e = wk.vortex_exact(wk.vortex(8, 2), X)
+    P = 0.4 * (e - 0.5 * (mx * mx + my * my) / rho)
+    assert np.allclose(P, rho ** 1.4, rtol=1e-13)
+    # far from the core the gas is at rest with rho = (gamma-1)^(1/(gamma-1)) * 1 ... = 0.4^2.5
+    assert abs(wk.vortex_exact(wk.vortex(8, 2), (np.array([5.0]), np.array([5.0])))[0][0] - 0.4 ** 2.5) < 1e-9

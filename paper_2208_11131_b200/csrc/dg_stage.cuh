@@ -439,25 +439,57 @@ __device__ __forceinline__ void wavespeed_points(const double *RA, double gamma,
     block_max2<NT>(cmax, vmax, red, maxbits, tid);
 }
 
-// Block -> tile map.  A tile is C consecutive cells of one x-row.  In 3D the tiles are visited in groups of 8 y-rows
-// x 8 z-planes (x fastest, then y within the group, then z within the group), so that the y and z neighbours of a
-// tile are at most 8 x-rows away in launch order and their rows (state for the face kernel, face fluxes for the
-// stage kernel) are still in L2 -- or in flight -- when they are read; 1/8 of the tiles per axis reach across a
-// group boundary.  Falls back to the natural order when the mesh does not divide (nx % C, ny % 8, nz % 8).
-template <int D, int C>
-__device__ __forceinline__ int tile_of_block(int b, int nx, int ny, int nz) {
-    if (D != 3 || (nx % C) != 0 || (ny % 8) != 0 || (nz % 8) != 0) return b;
-    const int ntx = nx / C;
-    const int gsz = ntx * 64;
-    const int gi = b / gsz;
-    int r = b - gi * gsz;
-    const int xb = r % ntx;
-    r /= ntx;
-    const int ngy = ny / 8;
-    const int iy = (gi % ngy) * 8 + (r % 8);
-    const int iz = (gi / ngy) * 8 + (r / 8);
-    return (iz * ny + iy) * ntx + xb;
+// Block -> tile map.  A tile is C consecutive cells of one x-row.  In 3D, when the mesh divides (nx % C, ny % 8,
+// nz % 8), the tiles are visited in groups of 8 y-rows x 8 z-planes (x fastest, then y within the group, then z within
+// the group), so that the y and z neighbours of a tile are at most 8 x-rows away in launch order and their rows (state
+// for the face kernel, face fluxes for the stage kernel) are still in L2 -- or in flight -- when they are read; 1/8 of
+// the tiles per axis reach across a group boundary.  That order is expressed as a 3D grid
+//     gridDim = (nx / C, 64 * (ny / 8), nz / 8),   blockIdx.y = 64 * (y group) + 8 * (z in group) + (y in group)
+// (blocks are issued x fastest, then y, then z), which gives every thread its (ix, iy, iz) without one integer
+// division: the generic 1D map (ragged meshes, tiles that straddle x-rows) costs ~300 instructions per warp.
+__host__ __device__ inline bool tile_grid_blocked(int D, int C, int nx, int ny, int nz) {
+    return D == 3 && (nx % C) == 0 && (ny % 8) == 0 && (nz % 8) == 0 && (ny / 8) * 64 <= 65535 && (nz / 8) <= 65535;
 }
+template <int D, int C>
+inline dim3 tile_grid(int ncells, int nx, int ny, int nz) {
+    if (tile_grid_blocked(D, C, nx, ny, nz)) return dim3(nx / C, 64 * (ny / 8), nz / 8);
+    return dim3((ncells + C - 1) / C, 1, 1);
+}
+// position of lane-cell `cl` of this block: first cell of the tile, clamped global cell index, coordinates
+template <int D, int C>
+struct TilePos {
+    int cell0, cg, ix, iy, iz;
+    bool active;
+    __device__ __forceinline__ TilePos(const DgStageArgs &p, int cl) {
+        if (D == 3 && gridDim.y > 1) {
+            const int r = blockIdx.y & 63;
+            iy = (blockIdx.y >> 6) * 8 + (r & 7);
+            iz = blockIdx.z * 8 + (r >> 3);
+            cell0 = (iz * p.ny + iy) * p.nx + blockIdx.x * C;
+            ix = blockIdx.x * C + cl;
+            cg = cell0 + cl;
+            active = true;
+        } else {
+            cell0 = blockIdx.x * C;
+            cg = min(cell0 + cl, p.ncells - 1);
+            active = cell0 + cl < p.ncells;
+            ix = cg % p.nx;
+            iy = (cg / p.nx) % p.ny;
+            iz = cg / (p.nx * p.ny);
+        }
+    }
+    // periodic neighbours: lower (-1) / upper (+1) along each axis
+    __device__ __forceinline__ int lower(const DgStageArgs &p, int a) const {
+        if (a == 0) return cg + ((ix == 0) ? p.nx - 1 : -1);
+        if (a == 1) return cg + ((iy == 0) ? (p.ny - 1) * p.nx : -p.nx);
+        return cg + ((iz == 0) ? (p.nz - 1) * p.nx * p.ny : -p.nx * p.ny);
+    }
+    __device__ __forceinline__ int upper(const DgStageArgs &p, int a) const {
+        if (a == 0) return cg + ((ix == p.nx - 1) ? 1 - p.nx : 1);
+        if (a == 1) return cg + ((iy == p.ny - 1) ? -(p.ny - 1) * p.nx : p.nx);
+        return cg + ((iz == p.nz - 1) ? -(p.nz - 1) * p.nx * p.ny : p.nx * p.ny);
+    }
+};
 
 // address of row `row` (compile-time multiple after unrolling) of a [row][cell] global array: one IMAD.WIDE
 __device__ __forceinline__ const double *row_ptr(const double *base, unsigned row, unsigned ncells) {
@@ -792,7 +824,8 @@ __global__ void __launch_bounds__(DG_FACE_NT, DG_FACE_MINB) dg_face_kernel(const
     int *nbr = reinterpret_cast<int *>(RX + K::NQ * K::Nf * C);
     double *bar = RX + K::NQ * K::Nf * C + (D * C + 1) / 2;   // mbarrier of the bulk copies, after nbr[D*C]
     const int tid = threadIdx.x;
-    const int cell0 = tile_of_block<D, C>(blockIdx.x, p.nx, p.ny, p.nz) * C;
+    const TilePos<D, C> pos(p, tid % C);
+    const int cell0 = pos.cell0;
     const bool bulk = bulk_ok<C>(cell0, p.ncells);
     if (bulk) {
         if (tid == 0) mbar_init(bar, 1);
@@ -800,21 +833,13 @@ __global__ void __launch_bounds__(DG_FACE_NT, DG_FACE_MINB) dg_face_kernel(const
         issue_own_modes_bulk<V, Np, C, NT, typename FK::LV>(p.w_prev, p.ncells, cell0, RA, bar, tid);
     }
     if (tid < C) {
-        const int c = min(cell0 + tid, p.ncells - 1);
-        const int ix = c % p.nx;
-        const int iy = (c / p.nx) % p.ny;
-        const int iz = c / (p.nx * p.ny);
-        nbr[0 * C + tid] = c + ((ix == p.nx - 1) ? 1 - p.nx : 1);
-        nbr[1 * C + tid] = c + ((iy == p.ny - 1) ? -(p.ny - 1) * p.nx : p.nx);
-        if (D == 3) {
-            const int pl = p.nx * p.ny;
-            nbr[(D - 1) * C + tid] = c + ((iz == p.nz - 1) ? -(p.nz - 1) * pl : pl);
-        }
+#pragma unroll
+        for (int a = 0; a < D; ++a) nbr[a * C + tid] = pos.upper(p, a);
     }
     if (bulk)
         mbar_wait(bar, 0);
     else
-        load_own_modes<V, Np, C, NT, typename FK::LV>(p.w_prev, p.ncells, min(cell0 + tid % C, p.ncells - 1), RA, tid);
+        load_own_modes<V, Np, C, NT, typename FK::LV>(p.w_prev, p.ncells, pos.cg, RA, tid);
     __syncthreads();
     face_axis<D, M, VISC, AV, 0>(p, RA, RX, nbr, cell0, tid);
     face_axis<D, M, VISC, AV, 1>(p, RA, RX, nbr, cell0, tid);

@@ -18,6 +18,16 @@
 
 #include "dg_stage.cuh"
 
+#ifndef DG_S2_NT3
+#define DG_S2_NT3 512
+#endif
+#ifndef DG_S2_CMAX3
+#define DG_S2_CMAX3 16
+#endif
+#ifndef DG_S2_MINB
+#define DG_S2_MINB 1
+#endif
+
 namespace dgk {
 
 template <int D, int M, bool VISC, bool AV>
@@ -26,15 +36,15 @@ struct Cfg2 {
     static constexpr int V = K::V, Vc = K::Vc, Np = K::Np, Nf = K::Nf;
     // one block of 16 warps per SM in 3D (measured: 128-byte rows of 16 cells beat two blocks of 8 cells at 128^3);
     // 2D tiles are small, several 8-warp blocks share an SM
-    static constexpr int NT = (D == 3) ? 512 : 256;
-    static constexpr int CMAX = (D == 3 && M >= 4) ? 16 : 32;
+    static constexpr int NT = (D == 3) ? DG_S2_NT3 : 256;
+    static constexpr int CMAX = (D == 3 && M >= 4) ? DG_S2_CMAX3 : 32;
     // doubles per cell: U (nodal values) + GR (gradients -> fluxes)
     static constexpr int FP = V * Np + D * Vc * Np;
     // Wk[c], wave-speed scratch, sensor partials, S table
     static constexpr int extra_doubles(int c) { return c + 2 * (NT / 32) + (AV ? 4 * (NT / 32) * c : 0) + M * M + 2; }
     static constexpr int pick_c() {
         int c = CMAX;
-        while (c > 1 && (c * FP + extra_doubles(c)) * 8 > 227 * 1024 - 1024) c >>= 1;
+        while (c > 1 && (c * FP + extra_doubles(c)) * 8 > (227 * 1024) / DG_S2_MINB - 1024) c >>= 1;
         return c;
     }
     static constexpr int C = pick_c();
@@ -44,7 +54,7 @@ struct Cfg2 {
 };
 
 template <int D, int M, bool VISC, bool AV>
-__global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), 1) dg_stage2_kernel(const DgStageArgs p) {
+__global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_stage2_kernel(const DgStageArgs p) {
     using K = Cfg<D, M, VISC, AV>;
     using K2 = Cfg2<D, M, VISC, AV>;
     constexpr int C = K2::C, NT = K2::NT, V = K::V, Vc = K::Vc, Np = K::Np, Nf = K::Nf;
@@ -68,19 +78,13 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), 1) dg_stage2_kerne
     const bool has_aux = p.w_aux != nullptr;
     if (tid < MM) sS[tid] = c_tab.S[(tid / M) * 8 + tid % M];
     {
-        const int tile = tile_of_block<D, C>(blockIdx.x, p.nx, p.ny, p.nz);
-        const int cell0 = tile * C;
-        const int cg = min(cell0 + cl, p.ncells - 1);
-        const bool active = cell0 + cl < p.ncells;
+        const TilePos<D, C> pos(p, cl);
+        const int cell0 = pos.cell0;
+        const int cg = pos.cg;
+        const bool active = pos.active;
         int nbm[D];                               // lower neighbour along each axis (periodic wrap)
-        {
-            const int ix = cg % p.nx;
-            const int iy = (cg / p.nx) % p.ny;
-            const int iz = cg / (p.nx * p.ny);
-            nbm[0] = cg + ((ix == 0) ? p.nx - 1 : -1);
-            nbm[1] = cg + ((iy == 0) ? (p.ny - 1) * p.nx : -p.nx);
-            if (D == 3) nbm[D - 1] = cg + ((iz == 0) ? (p.nz - 1) * p.nx * p.ny : -p.nx * p.ny);
-        }
+#pragma unroll
+        for (int a = 0; a < D; ++a) nbm[a] = pos.lower(p, a);
         if (AV && tid < C) {
             // wiggle source of Eq. 45 from the previous step's sensor (readings A14, A15)
             const int c = min(cell0 + tid, p.ncells - 1);

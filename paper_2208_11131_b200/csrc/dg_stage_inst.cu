@@ -48,8 +48,8 @@ cudaError_t launch(const DgStageArgs &a, cudaStream_t st, int wavespeed_only) {
     }
     if (wavespeed_only != 3) {
         using FK = dgk::FaceCfg<DG_DIM, DG_M, VISC, AV>;
-        const int fblocks = (a.ncells + FK::C - 1) / FK::C;
-        dgk::dg_face_kernel<DG_DIM, DG_M, VISC, AV><<<fblocks, FK::NT, FK::kSmemBytes, st>>>(a);
+        const dim3 fgrid = dgk::tile_grid<DG_DIM, FK::C>(a.ncells, a.nx, a.ny, a.nz);
+        dgk::dg_face_kernel<DG_DIM, DG_M, VISC, AV><<<fgrid, FK::NT, FK::kSmemBytes, st>>>(a);
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
@@ -57,8 +57,8 @@ cudaError_t launch(const DgStageArgs &a, cudaStream_t st, int wavespeed_only) {
         if constexpr (K::PP) {
             // register-tile configurations (2 <= m <= 5): second-generation stage kernel (dg_stage2.cuh)
             using K2 = dgk::Cfg2<DG_DIM, DG_M, VISC, AV>;
-            const int blocks2 = (a.ncells + K2::C - 1) / K2::C;
-            dgk::dg_stage2_kernel<DG_DIM, DG_M, VISC, AV><<<blocks2, K2::NT, K2::kSmemBytes, st>>>(a);
+            const dim3 grid2 = dgk::tile_grid<DG_DIM, K2::C>(a.ncells, a.nx, a.ny, a.nz);
+            dgk::dg_stage2_kernel<DG_DIM, DG_M, VISC, AV><<<grid2, K2::NT, K2::kSmemBytes, st>>>(a);
         } else {
             dgk::dg_stage_kernel<DG_DIM, DG_M, VISC, AV><<<blocks, K::NT, K::kSmemBytes, st>>>(a);
         }

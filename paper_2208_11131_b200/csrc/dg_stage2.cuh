@@ -27,6 +27,15 @@
 #ifndef DG_S2_MINB
 #define DG_S2_MINB 1
 #endif
+#ifndef DG_S2_PREFETCH
+#define DG_S2_PREFETCH 1
+#endif
+#ifndef DG_S2_UNROLL_E
+#define DG_S2_UNROLL_E 2
+#endif
+#ifndef DG_S2_UNROLL_B
+#define DG_S2_UNROLL_B 3
+#endif
 
 namespace dgk {
 
@@ -53,13 +62,16 @@ struct Cfg2 {
     static_assert(NT % C == 0, "threads per block must be a multiple of cells per block");
 };
 
-template <int D, int M, bool VISC, bool AV>
+// PLAIN: the RK-stage form every time step uses (not rhs_only, full tensor basis, no SSPRK(5,4) auxiliary row): those
+// three switches become compile-time constants, which removes their selects from the combine loops.
+template <int D, int M, bool VISC, bool AV, bool PLAIN>
 __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_stage2_kernel(const DgStageArgs p) {
     using K = Cfg<D, M, VISC, AV>;
     using K2 = Cfg2<D, M, VISC, AV>;
     constexpr int C = K2::C, NT = K2::NT, V = K::V, Vc = K::Vc, Np = K::Np, Nf = K::Nf;
     constexpr bool GRAD = K::GRAD;
     constexpr int MM = M * M;
+    constexpr int kUnrollE = DG_S2_UNROLL_E, kUnrollB = DG_S2_UNROLL_B;
     constexpr int NTILE = Np / MM;               // m x m tiles per slot (m in 3D, 1 in 2D)
     using L = Lay<MM, Np, use_swizzle(M, C), 0>;
     extern __shared__ __align__(128) double smem[];
@@ -73,9 +85,13 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
     const int cl = tid % C;
     const double ih = 1.0 / p.h;
     const double pref = (D == 3 ? 0.25 : 0.5) * ih;
-    const double cdt = p.rhs_only ? 1.0 : p.rk_c * p.scal[0];
-    const bool need_n = !p.rhs_only, need_p = !p.rhs_only && p.rk_b != 0.0;
-    const bool has_aux = p.w_aux != nullptr;
+    const bool rhs_only = PLAIN ? false : (p.rhs_only != 0);
+    const bool total_degree = PLAIN ? false : (p.total_degree != 0);
+    const bool has_aux = PLAIN ? false : (p.w_aux != nullptr);
+    const double cdt = rhs_only ? 1.0 : p.rk_c * p.scal[0];
+    const bool need_n = !rhs_only, need_p = !rhs_only && p.rk_b != 0.0;
+    const double cdtp = cdt * pref;
+    const bool sens_stage = p.do_sensor != 0;
     if (tid < MM) sS[tid] = c_tab.S[(tid / M) * 8 + tid % M];
     {
         const TilePos<D, C> pos(p, cl);
@@ -101,6 +117,12 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
             const double *src = p.w_prev + (size_t)(lz * MM * V + v) * p.ncells + cg;
 #pragma unroll
             for (int q = 0; q < MM; ++q) t[q] = __ldg(row_ptr(src, q * V, p.ncells));
+            if (DG_S2_PREFETCH && D == 3 && need_n && p.w_n != p.w_prev && (cl & 3) == 0) {
+                // u^n is read by the stage combine only (phase H): start its rows towards L2 now (one request per sector)
+                const double *pn = p.w_n + (size_t)(lz * MM * V + v) * p.ncells + cg;
+#pragma unroll
+                for (int q = 0; q < MM; ++q) asm volatile("prefetch.global.L2 [%0];" ::"l"(row_ptr(pn, q * V, p.ncells)));
+            }
             tile_x<DG_SEL_V, M>(t);
             tile_y<DG_SEL_V, M>(t);
             tile_store<M, C, L>(U, g, cl, t);
@@ -121,28 +143,24 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
         __syncthreads();
         if (D == 3) {
             // ---- B: expansion along z, z derivative ----
-            for (int it = tid; it < V * MM * C; it += NT) {
+            constexpr int NKB = (V * MM * C + NT - 1) / NT;
+#pragma unroll kUnrollB
+            for (int kb = 0; kb < NKB; ++kb) {
+                const int it = tid + kb * NT;
+                if (it >= V * MM * C) break;
                 const int r = it / C;
                 const int q = r % MM, v = r / MM;
                 double in[M], u[M];
 #pragma unroll
                 for (int l = 0; l < M; ++l) in[l] = U[L::at2(v, q + l * MM) * C + cl];
+                apply1d<DG_SEL_V, M>(in, u);
 #pragma unroll
-                for (int j = 0; j < M; ++j) {
-                    double acc = c_tab.V[j * 8] * in[0];
-#pragma unroll
-                    for (int l = 1; l < M; ++l) acc = fma(c_tab.V[j * 8 + l], in[l], acc);
-                    u[j] = acc;
-                    U[L::at2(v, q + j * MM) * C + cl] = acc;
-                }
+                for (int j = 0; j < M; ++j) U[L::at2(v, q + j * MM) * C + cl] = u[j];
                 if (GRAD && v < Vc) {
+                    double gz[M];
+                    apply1d<DG_SEL_DHAT, M>(u, gz);
 #pragma unroll
-                    for (int j = 0; j < M; ++j) {
-                        double acc = c_tab.Dhat[j * 8] * u[0];
-#pragma unroll
-                        for (int i = 1; i < M; ++i) acc = fma(c_tab.Dhat[j * 8 + i], u[i], acc);
-                        GR[L::at2(2 * Vc + v, q + j * MM) * C + cl] = acc * (2.0 * ih);
-                    }
+                    for (int j = 0; j < M; ++j) GR[L::at2(2 * Vc + v, q + j * MM) * C + cl] = gz[j] * (2.0 * ih);
                 }
             }
             __syncthreads();
@@ -171,7 +189,11 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
             bool bad = false;
             double amax = 0.0;                                     // max alpha at the Gauss points (diagnostics)
             const double decay = (double)M / (p.f_tau * p.h);      // 1/tau = (n+1) c_s / (f_tau h), Eq. 44
-            for (int it = tid; it < Np * C; it += NT) {
+            constexpr int NKE = (Np * C + NT - 1) / NT;
+#pragma unroll kUnrollE
+            for (int ke = 0; ke < NKE; ++ke) {
+                const int it = tid + ke * NT;
+                if (it >= Np * C) break;
                 const int j = it / C;
                 double u[Vc];
 #pragma unroll
@@ -279,13 +301,13 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
                 for (int y = 0; y < M; ++y)
 #pragma unroll
                     for (int x = 0; x < M; ++x)
-                        n[y * M + x] += c_tab.Pend[0][x] * gf[k][1][y] - c_tab.Pend[1][x] * gf[k][0][y];
+                        n[y * M + x] = fma(-c_tab.Pend[1][x], gf[k][0][y], fma(c_tab.Pend[0][x], gf[k][1][y], n[y * M + x]));
                 tile_y<DG_SEL_VTG, M>(n);
 #pragma unroll
                 for (int y = 0; y < M; ++y)
 #pragma unroll
                     for (int x = 0; x < M; ++x)
-                        n[y * M + x] += c_tab.Pend[0][y] * gf[k][3][x] - c_tab.Pend[1][y] * gf[k][2][x];
+                        n[y * M + x] = fma(-c_tab.Pend[1][y], gf[k][2][x], fma(c_tab.Pend[0][y], gf[k][3][x], n[y * M + x]));
             } else {
                 tile_load<M, C, L>(U, g, cl, n);      // alpha source (slot Vc of U)
                 tile_x<DG_SEL_VTG, M>(n);
@@ -306,17 +328,17 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
                 }
 #pragma unroll
                 for (int q = 0; q < MM; ++q) {
-                    const bool keep = !p.total_degree || (q % M + q / M <= M - 1);
+                    const bool keep = !total_degree || (q % M + q / M <= M - 1);
                     const double Ld = keep ? pref * n[q] : 0.0;
                     double wnew = Ld;
-                    if (!p.rhs_only) wnew = fma(cdt, Ld, fma(p.rk_b, wp[q], p.rk_a * wn[q]));
+                    if (!rhs_only) wnew = fma(cdt, Ld, fma(p.rk_b, wp[q], p.rk_a * wn[q]));
                     if (active) *row_ptr(bo, q * V, p.ncells) = wnew;
                     if (has_aux && active) {
                         const size_t gi = (size_t)(q * V + v) * p.ncells + cg;
                         p.w_aux[gi] = fma(p.aux_c * p.scal[0], Ld, fma(p.aux_b, wp[q], p.aux_a * p.w_aux_in[gi]));
                     }
                     if (AV && p.do_sensor && v == 0) {
-                        const bool top = p.total_degree ? (q % M + q / M == M - 1) : ((q % M == M - 1) || (q / M == M - 1));
+                        const bool top = total_degree ? (q % M + q / M == M - 1) : ((q % M == M - 1) || (q / M == M - 1));
                         sB = fma(wn[q], wn[q], sB);
                         dB = fma(wn[q], Ld, dB);
                         if (top) {
@@ -373,17 +395,24 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
                 for (int j = 0; j < M; ++j) in[j] = U[L::at2(v, q + j * MM) * C + cl];
                 const bool topxy = (q % M == M - 1) || (q / M == M - 1);
                 const int lxy = q % M + q / M;
+                double pz[M];
+                apply1d<DG_SEL_VTG, M>(in, pz);
 #pragma unroll
                 for (int l = 0; l < M; ++l) {
-                    double acc = c_tab.VtG[l * 8] * in[0];
-#pragma unroll
-                    for (int j = 1; j < M; ++j) acc = fma(c_tab.VtG[l * 8 + j], in[j], acc);
-                    if (v < Vc) acc += c_tab.Pend[0][l] * hfz[k][1] - c_tab.Pend[1][l] * hfz[k][0];
+                    double acc = pz[l];
+                    if (v < Vc) acc = fma(-c_tab.Pend[1][l], hfz[k][0], fma(c_tab.Pend[0][l], hfz[k][1], acc));
                     // total-degree basis: the discarded modes are not test functions of Eq. 20
-                    const bool keep = !p.total_degree || (lxy + l <= M - 1);
-                    const double Ld = keep ? pref * acc : 0.0;
-                    double wnew = Ld;
-                    if (!p.rhs_only) wnew = fma(cdt, Ld, fma(p.rk_b, hwp[k][l], p.rk_a * hwn[k][l]));
+                    const bool keep = !total_degree || (lxy + l <= M - 1);
+                    double Ld, wnew;
+                    if (PLAIN) {
+                        // prefactor folded into the combine; dw/dt itself is needed by the sensor sums only
+                        wnew = fma(cdtp, acc, fma(p.rk_b, hwp[k][l], p.rk_a * hwn[k][l]));
+                        Ld = (AV && sens_stage) ? pref * acc : 0.0;
+                    } else {
+                        Ld = keep ? pref * acc : 0.0;
+                        wnew = Ld;
+                        if (!rhs_only) wnew = fma(cdt, Ld, fma(p.rk_b, hwp[k][l], p.rk_a * hwn[k][l]));
+                    }
                     if (active) *row_ptr(bo, l * MM * V, p.ncells) = wnew;
                     if (has_aux && active) {
                         const size_t gi = (size_t)((l * MM + q) * V + v) * p.ncells + cg;
@@ -392,7 +421,7 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
                     if (AV && p.do_sensor && v == 0) {
                         sB = fma(hwn[k][l], hwn[k][l], sB);
                         dB = fma(hwn[k][l], Ld, dB);
-                        if (p.total_degree ? (lxy + l == M - 1) : (topxy || l == M - 1)) {
+                        if (total_degree ? (lxy + l == M - 1) : (topxy || l == M - 1)) {
                             sA = fma(hwn[k][l], hwn[k][l], sA);
                             dA = fma(hwn[k][l], Ld, dA);
                         }

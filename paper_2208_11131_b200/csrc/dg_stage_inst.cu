@@ -22,7 +22,11 @@ cudaError_t configure() {
     // NB: a kernel template must only ever be instantiated in the translation unit of its own (dim, m): every unit
     // has its own __constant__ tables, and the host stubs of equal instantiations are merged by the linker
     if constexpr (K::PP) {
-        e = cudaFuncSetAttribute(dgk::dg_stage2_kernel<DG_DIM, DG_M, VISC, AV>,
+        e = cudaFuncSetAttribute(dgk::dg_stage2_kernel<DG_DIM, DG_M, VISC, AV, false>,
+                                 cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 dgk::Cfg2<DG_DIM, DG_M, VISC, AV>::kSmemBytes);
+        if (e != cudaSuccess) return e;
+        e = cudaFuncSetAttribute(dgk::dg_stage2_kernel<DG_DIM, DG_M, VISC, AV, true>,
                                  cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  dgk::Cfg2<DG_DIM, DG_M, VISC, AV>::kSmemBytes);
         if (e != cudaSuccess) return e;
@@ -58,7 +62,10 @@ cudaError_t launch(const DgStageArgs &a, cudaStream_t st, int wavespeed_only) {
             // register-tile configurations (2 <= m <= 5): second-generation stage kernel (dg_stage2.cuh)
             using K2 = dgk::Cfg2<DG_DIM, DG_M, VISC, AV>;
             const dim3 grid2 = dgk::tile_grid<DG_DIM, K2::C>(a.ncells, a.nx, a.ny, a.nz);
-            dgk::dg_stage2_kernel<DG_DIM, DG_M, VISC, AV><<<grid2, K2::NT, K2::kSmemBytes, st>>>(a);
+            if (!a.rhs_only && !a.total_degree && a.w_aux == nullptr)
+                dgk::dg_stage2_kernel<DG_DIM, DG_M, VISC, AV, true><<<grid2, K2::NT, K2::kSmemBytes, st>>>(a);
+            else
+                dgk::dg_stage2_kernel<DG_DIM, DG_M, VISC, AV, false><<<grid2, K2::NT, K2::kSmemBytes, st>>>(a);
         } else {
             dgk::dg_stage_kernel<DG_DIM, DG_M, VISC, AV><<<blocks, K::NT, K::kSmemBytes, st>>>(a);
         }

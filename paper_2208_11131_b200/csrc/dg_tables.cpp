@@ -92,6 +92,16 @@ void dg_build_tables(int m, DgTables *t) {
             t->VtG[l * 8 + j] = (double)(V[j][l] * g[j]);
         }
     }
+    // even-odd forms of the two nodal -> nodal matrices (dg_stage.cuh apply1d): half-sums / half-differences of the
+    // mirrored columns, formed in long double
+    for (int j = 0; j < m; ++j)
+        for (int i = 0; i < m / 2; ++i) {
+            const ld sji = Dh[i][j] * g[i] / g[j], sjm = Dh[m - 1 - i][j] * g[m - 1 - i] / g[j];
+            t->DhatE[j * 8 + i] = (double)(0.5L * (Dh[j][i] + Dh[j][m - 1 - i]));
+            t->DhatO[j * 8 + i] = (double)(0.5L * (Dh[j][i] - Dh[j][m - 1 - i]));
+            t->SE[j * 8 + i] = (double)(0.5L * (sji + sjm));
+            t->SO[j * 8 + i] = (double)(0.5L * (sji - sjm));
+        }
     {
         ld P[DG_MAXM + 2], dP[DG_MAXM + 2];
         legendre_norm(n, -1.0L, P, dP);

@@ -15,6 +15,10 @@ struct DgTables {
     double Dhat[DG_MAXM * 8];  // Dhat[j][i]= (D V^-1)[j][i]               nodal -> d/dxi at the nodes
     double S[DG_MAXM * 8];     // S[j'][j]  = Dhat[j][j'] g_j / g_j'       weak-form derivative, nodal -> nodal
     double VtG[DG_MAXM * 8];   // VtG[l][j] = P_l(x_j) g_j                 weighted nodal -> modal projection
+    double DhatE[DG_MAXM * 8]; // (Dhat[j][i] + Dhat[j][m-1-i]) / 2, i < m/2   even-odd form of Dhat (centro-antisymmetric)
+    double DhatO[DG_MAXM * 8]; // (Dhat[j][i] - Dhat[j][m-1-i]) / 2
+    double SE[DG_MAXM * 8];    // same for S
+    double SO[DG_MAXM * 8];
     double Pend[2][8];         // P_l(-1), P_l(+1)                         face traces
     double Rv[2][8];           // R^-_l (left cell), R^+_l (right cell)    recovered interface value
     double Gv[2][8];           // G^-_l, G^+_l                             recovered interface normal derivative * h

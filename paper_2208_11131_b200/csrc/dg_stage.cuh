@@ -42,8 +42,11 @@
 #ifndef DG_FACE_NT
 #define DG_FACE_NT 256
 #endif
-#ifndef DG_FACE_PREFETCH
-#define DG_FACE_PREFETCH 1
+#ifndef DG_FACE_DIRECT
+#define DG_FACE_DIRECT 1
+#endif
+#ifndef DG_FACE_DIRECT_MINB
+#define DG_FACE_DIRECT_MINB 3
 #endif
 #ifndef DG_FACE_MINB
 #define DG_FACE_MINB 2
@@ -295,6 +298,16 @@ __device__ __forceinline__ void tile_y(double *t) {
 #pragma unroll
         for (int j = 0; j < M; ++j) t[j * M + x] = res[j];
     }
+}
+// acc += (MAT along y) t, plain form (no separate add pass)
+template <int SEL, int M>
+__device__ __forceinline__ void tile_y_acc(const double *t, double *acc) {
+#pragma unroll
+    for (int x = 0; x < M; ++x)
+#pragma unroll
+        for (int j = 0; j < M; ++j)
+#pragma unroll
+            for (int i = 0; i < M; ++i) acc[j * M + x] = fma(mat<SEL>(j * 8 + i), t[i * M + x], acc[j * M + x]);
 }
 // tile g (global plane index: P = g*M*M + q) of an array <-> registers; L::PL must be M*M
 template <int M, int C, class L>
@@ -661,10 +674,16 @@ template <int D, int M, bool VISC, bool AV>
 struct FaceCfg {
     using K = Cfg<D, M, VISC, AV>;
     static constexpr int NT = DG_FACE_NT;
-    static constexpr int FP = K::V * K::Np + K::NQ * K::Nf;       // doubles per cell: own modes + one face
+    // DIRECT (3D register-tile configurations): F1 reads the own modes straight from global memory / L1 like the
+    // neighbour's (each is used once per axis), so no copy of the tile is staged in shared memory, the block does
+    // not wait for it before the first axis, and only the face scratch remains (more cells or blocks per SM)
+    static constexpr bool DIRECT = DG_FACE_DIRECT && K::BLK && (D == 3);
+    static constexpr int FP = (DIRECT ? 0 : K::V * K::Np) + K::NQ * K::Nf;   // doubles per cell: [own modes +] one face
+    static constexpr int MINB = DIRECT ? DG_FACE_DIRECT_MINB : DG_FACE_MINB;   // resident blocks per SM (register cap)
+    static constexpr int CMAX = DIRECT ? 16 : 32;
     static constexpr int pick_c() {
-        int c = 32;
-        while (c > 1 && c * FP * 8 > (227 * 1024) / DG_FACE_MINB - 2048) c >>= 1;   // DG_FACE_MINB resident blocks per SM
+        int c = CMAX;
+        while (c > 1 && c * FP * 8 > (227 * 1024) / MINB - 2048) c >>= 1;   // MINB resident blocks per SM
         return c;
     }
     static constexpr int C = pick_c();
@@ -694,55 +713,66 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA
     {
         static_assert(NT % C == 0, "threads per block must be a multiple of cells per block");
         constexpr int NIT = (V * Nf * C + NT - 1) / NT;
+        constexpr int NB = FK::DIRECT ? (NIT % 3 == 0 ? 3 : (NIT % 2 == 0 ? 2 : 1)) : NIT;   // items per load batch
         const int cell = tid % C;
         const int nc = nbr[A * C + cell];
-        double nb[NIT][M];
+        const int oc = min(cell0 + cell, p.ncells - 1);
         // the upper x neighbour of every cell but the last one of the tile is the next cell of the tile itself
-        const bool from_tile = (A == 0) && (cell < C - 1) && (cell0 + cell + 1 < p.ncells) && (nc == cell0 + cell + 1);
+        const bool from_tile = !FK::DIRECT && (A == 0) && (cell < C - 1) && (cell0 + cell + 1 < p.ncells) &&
+                               (nc == cell0 + cell + 1);
 #pragma unroll
-        for (int k = 0; k < NIT; ++k) {
-            const int r = tid / C + k * (NT / C);          // v*Nf + lt
-            if (r < V * Nf) {
-                const int base = pencil_base<M, SA>(r % Nf);
-                const int v = r / Nf;
-                if (from_tile) {
+        for (int k0 = 0; k0 < NIT; k0 += NB) {
+            double nb[NB][M], ow[NB][M];
 #pragma unroll
-                    for (int l = 0; l < M; ++l) nb[k][l] = RA[LV::at2(v, base + l * SA) * C + cell + 1];
-                } else {
+            for (int kk = 0; kk < NB; ++kk) {
+                const int r = tid / C + (k0 + kk) * (NT / C);          // v*Nf + lt
+                if (r < V * Nf) {
+                    const int base = pencil_base<M, SA>(r % Nf);
+                    const int v = r / Nf;
+                    if (from_tile) {
 #pragma unroll
-                    for (int l = 0; l < M; ++l)
-                        nb[k][l] = __ldg(p.w_prev + (size_t)((base + l * SA) * V + v) * p.ncells + nc);
-                }
-            }
-        }
+                        for (int l = 0; l < M; ++l) nb[kk][l] = RA[LV::at2(v, base + l * SA) * C + cell + 1];
+                    } else {
 #pragma unroll
-        for (int k = 0; k < NIT; ++k) {
-            const int r = tid / C + k * (NT / C);
-            if (r < V * Nf) {
-                const int lt = r % Nf;
-                const int v = r / Nf;
-                const int base = pencil_base<M, SA>(lt);
-                double own[M];
+                        for (int l = 0; l < M; ++l)
+                            nb[kk][l] = __ldg(p.w_prev + (size_t)((base + l * SA) * V + v) * p.ncells + nc);
+                    }
+                    if (FK::DIRECT) {
 #pragma unroll
-                for (int l = 0; l < M; ++l) own[l] = RA[LV::at2(v, base + l * SA) * C + cell];
-                double uL = 0.0, uR = 0.0, ut = 0.0, gn = 0.0;
-#pragma unroll
-                for (int l = 0; l < M; ++l) {
-                    uL = fma(c_tab.Pend[1][l], own[l], uL);
-                    uR = fma(c_tab.Pend[0][l], nb[k][l], uR);
-                    if (GRAD) {
-                        ut = fma(c_tab.Rv[0][l], own[l], ut);
-                        ut = fma(c_tab.Rv[1][l], nb[k][l], ut);
-                        gn = fma(c_tab.Gv[0][l], own[l], gn);
-                        gn = fma(c_tab.Gv[1][l], nb[k][l], gn);
+                        for (int l = 0; l < M; ++l)
+                            ow[kk][l] = __ldg(p.w_prev + (size_t)((base + l * SA) * V + v) * p.ncells + oc);
                     }
                 }
-                if (v < Vc) {
-                    RX[LF::at2(oUL + v, lt) * C + cell] = uL;
-                    RX[LF::at2(oUR + v, lt) * C + cell] = uR;
-                    if (GRAD) RX[LF::at2(oGN + v, lt) * C + cell] = gn * ih;
+            }
+#pragma unroll
+            for (int kk = 0; kk < NB; ++kk) {
+                const int r = tid / C + (k0 + kk) * (NT / C);
+                if (r < V * Nf) {
+                    const int lt = r % Nf;
+                    const int v = r / Nf;
+                    const int base = pencil_base<M, SA>(lt);
+                    double own[M];
+#pragma unroll
+                    for (int l = 0; l < M; ++l) own[l] = FK::DIRECT ? ow[kk][l] : RA[LV::at2(v, base + l * SA) * C + cell];
+                    double uL = 0.0, uR = 0.0, ut = 0.0, gn = 0.0;
+#pragma unroll
+                    for (int l = 0; l < M; ++l) {
+                        uL = fma(c_tab.Pend[1][l], own[l], uL);
+                        uR = fma(c_tab.Pend[0][l], nb[kk][l], uR);
+                        if (GRAD) {
+                            ut = fma(c_tab.Rv[0][l], own[l], ut);
+                            ut = fma(c_tab.Rv[1][l], nb[kk][l], ut);
+                            gn = fma(c_tab.Gv[0][l], own[l], gn);
+                            gn = fma(c_tab.Gv[1][l], nb[kk][l], gn);
+                        }
+                    }
+                    if (v < Vc) {
+                        RX[LF::at2(oUL + v, lt) * C + cell] = uL;
+                        RX[LF::at2(oUR + v, lt) * C + cell] = uR;
+                        if (GRAD) RX[LF::at2(oGN + v, lt) * C + cell] = gn * ih;
+                    }
+                    if (GRAD) RX[LF::at2(oUT + v, lt) * C + cell] = ut;
                 }
-                if (GRAD) RX[LF::at2(oUT + v, lt) * C + cell] = ut;
             }
         }
     }
@@ -891,19 +921,19 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA
 }
 
 template <int D, int M, bool VISC, bool AV>
-__global__ void __launch_bounds__(DG_FACE_NT, DG_FACE_MINB) dg_face_kernel(const DgStageArgs p) {
+__global__ void __launch_bounds__(DG_FACE_NT, (FaceCfg<D, M, VISC, AV>::MINB)) dg_face_kernel(const DgStageArgs p) {
     using K = Cfg<D, M, VISC, AV>;
     using FK = FaceCfg<D, M, VISC, AV>;
     constexpr int C = FK::C, NT = FK::NT, V = K::V, Np = K::Np;
     extern __shared__ __align__(128) double smem[];
     double *RA = smem;
-    double *RX = RA + V * Np * C;
+    double *RX = RA + (FK::DIRECT ? 0 : V * Np * C);
     int *nbr = reinterpret_cast<int *>(RX + K::NQ * K::Nf * C);
     double *bar = RX + K::NQ * K::Nf * C + (D * C + 1) / 2;   // mbarrier of the bulk copies, after nbr[D*C]
     const int tid = threadIdx.x;
     const TilePos<D, C> pos(p, tid % C);
     const int cell0 = pos.cell0;
-    const bool bulk = bulk_ok<C>(cell0, p.ncells);
+    const bool bulk = !FK::DIRECT && bulk_ok<C>(cell0, p.ncells);
     if (bulk) {
         if (tid == 0) mbar_init(bar, 1);
         __syncthreads();
@@ -913,20 +943,9 @@ __global__ void __launch_bounds__(DG_FACE_NT, DG_FACE_MINB) dg_face_kernel(const
 #pragma unroll
         for (int a = 0; a < D; ++a) nbr[a * C + tid] = pos.upper(p, a);
     }
-    if (DG_FACE_PREFETCH && D == 3) {
-        // the upper y and z neighbours' modes are first touched by this block (their own blocks run later in the
-        // (y,z)-blocked order): start them towards L2 now, behind the x axis (one request per 32-byte sector)
-        constexpr int SEG = (C + 3) / 4;
-        const int ny_ = pos.upper(p, 1) - (tid % C), nz_ = pos.upper(p, 2) - (tid % C);
-        for (int i = tid; i < 2 * V * Np * SEG; i += NT) {
-            const int seg = i % SEG, r = (i / SEG) % (V * Np), which = i / (SEG * V * Np);
-            const double *q = p.w_prev + (size_t)r * p.ncells + (which ? nz_ : ny_) + seg * 4;
-            asm volatile("prefetch.global.L2 [%0];" ::"l"(q));
-        }
-    }
     if (bulk)
         mbar_wait(bar, 0);
-    else
+    else if (!FK::DIRECT)
         load_own_modes<V, Np, C, NT, typename FK::LV>(p.w_prev, p.ncells, pos.cg, RA, tid);
     __syncthreads();
     face_axis<D, M, VISC, AV, 0>(p, RA, RX, nbr, cell0, tid);

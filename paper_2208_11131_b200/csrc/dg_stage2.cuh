@@ -27,9 +27,6 @@
 #ifndef DG_S2_MINB
 #define DG_S2_MINB 1
 #endif
-#ifndef DG_S2_PREFETCH
-#define DG_S2_PREFETCH 1
-#endif
 #ifndef DG_S2_UNROLL_E
 #define DG_S2_UNROLL_E 2
 #endif
@@ -117,12 +114,6 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
             const double *src = p.w_prev + (size_t)(lz * MM * V + v) * p.ncells + cg;
 #pragma unroll
             for (int q = 0; q < MM; ++q) t[q] = __ldg(row_ptr(src, q * V, p.ncells));
-            if (DG_S2_PREFETCH && D == 3 && need_n && p.w_n != p.w_prev && (cl & 3) == 0) {
-                // u^n is read by the stage combine only (phase H): start its rows towards L2 now (one request per sector)
-                const double *pn = p.w_n + (size_t)(lz * MM * V + v) * p.ncells + cg;
-#pragma unroll
-                for (int q = 0; q < MM; ++q) asm volatile("prefetch.global.L2 [%0];" ::"l"(row_ptr(pn, q * V, p.ncells)));
-            }
             tile_x<DG_SEL_V, M>(t);
             tile_y<DG_SEL_V, M>(t);
             tile_store<M, C, L>(U, g, cl, t);
@@ -131,12 +122,8 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
 #pragma unroll
                 for (int q = 0; q < MM; ++q) a[q] = t[q];
                 tile_x<DG_SEL_DHAT, M>(a);
-#pragma unroll
-                for (int q = 0; q < MM; ++q) a[q] *= 2.0 * ih;
                 tile_store<M, C, L>(GR, g, cl, a);
                 tile_y<DG_SEL_DHAT, M>(t);
-#pragma unroll
-                for (int q = 0; q < MM; ++q) t[q] *= 2.0 * ih;
                 tile_store<M, C, L>(GR, Vc * NTILE + g, cl, t);
             }
         }
@@ -160,7 +147,7 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
                     double gz[M];
                     apply1d<DG_SEL_DHAT, M>(u, gz);
 #pragma unroll
-                    for (int j = 0; j < M; ++j) GR[L::at2(2 * Vc + v, q + j * MM) * C + cl] = gz[j] * (2.0 * ih);
+                    for (int j = 0; j < M; ++j) GR[L::at2(2 * Vc + v, q + j * MM) * C + cl] = gz[j];
                 }
             }
             __syncthreads();
@@ -173,12 +160,8 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
 #pragma unroll
                     for (int q = 0; q < MM; ++q) a[q] = t[q];
                     tile_x<DG_SEL_DHAT, M>(a);
-#pragma unroll
-                    for (int q = 0; q < MM; ++q) a[q] *= 2.0 * ih;
                     tile_store<M, C, L>(GR, g, cl, a);
                     tile_y<DG_SEL_DHAT, M>(t);
-#pragma unroll
-                    for (int q = 0; q < MM; ++q) t[q] *= 2.0 * ih;
                     tile_store<M, C, L>(GR, Vc * NTILE + g, cl, t);
                 }
                 __syncthreads();
@@ -200,14 +183,22 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
                 for (int v = 0; v < Vc; ++v) u[v] = U[L::at2(v, j) * C + cl];
                 const Prim<D> q = primitives<D>(u, p.gamma);
                 bad |= !(q.rho > 0.0) || !(q.p > 0.0);
+                // the gradient arrays hold d/dxi (reference coordinates): the factor 2/h of the cell map is folded
+                // into the two scalars that multiply them, 1/rho (velocity and temperature gradients) and eps
                 double g[D][D + 2], dv[D][D];
-                double divv = 0.0, eps = 0.0;
+                double divv = 0.0, epss = 0.0;
+                const double gs = 2.0 * ih;
+                const double irs = q.ir * gs;
                 if (GRAD) {
 #pragma unroll
                     for (int b = 0; b < D; ++b)
 #pragma unroll
                         for (int v = 0; v < Vc; ++v) g[b][v] = GR[L::at2(b * Vc + v, j) * C + cl];
-                    velocity_gradient<D>(q, g, dv);
+                    // dv[b][c] = d v_c / d x_b = (d_b(rho v_c) - v_c d_b rho) / rho
+#pragma unroll
+                    for (int b = 0; b < D; ++b)
+#pragma unroll
+                        for (int c = 0; c < D; ++c) dv[b][c] = (g[b][1 + c] - q.v[c] * g[b][0]) * irs;
 #pragma unroll
                     for (int b = 0; b < D; ++b) divv += dv[b][b];
                 }
@@ -215,19 +206,49 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
                     const double al = U[L::at2(Vc, j) * C + cl];
                     const double cs = fast_sqrt(p.gamma * q.p * q.ir);
                     if (active) amax = fmax(amax, al);
-                    eps = fmin(fmax(al, 0.0), p.alpha_max) * cs * (p.h / (double)M);        // Eq. 46, A17
+                    epss = fmin(fmax(al, 0.0), p.alpha_max) * cs * (p.h / (double)M) * gs;        // Eq. 46, A17
                     // Eq. 43-45: shock source + wiggle source - decay; stored pre-scaled by h/2 for the projection
                     const double src = p.f_v * fmax(0.0, -divv) + Wk[cl] - al * (cs * decay);
                     U[L::at2(Vc, j) * C + cl] = 0.5 * p.h * src;
+                }
+                // Navier-Stokes stress (Eq. 38-39, traceless Pi, reading A7): symmetric, formed once for the D axes
+                double Pi[D][D], qh[D];
+                if (VISC) {
+                    const double mu = p.nu * q.rho, kq = p.chi * (p.gamma - 1.0) * q.rho;
+                    const double tt = (2.0 / 3.0) * divv, eir = q.e * q.ir;
+#pragma unroll
+                    for (int a = 0; a < D; ++a) {
+#pragma unroll
+                        for (int b = a; b < D; ++b) {
+                            Pi[a][b] = mu * (dv[a][b] + dv[b][a] - (a == b ? tt : 0.0));
+                            Pi[b][a] = Pi[a][b];
+                        }
+                    }
+#pragma unroll
+                    for (int a = 0; a < D; ++a) {
+                        // chi (gamma-1) rho d_a u_th,  u_th = e/rho - v^2/2
+                        double vdv = 0.0;
+#pragma unroll
+                        for (int c = 0; c < D; ++c) vdv = fma(q.v[c], dv[a][c], vdv);
+                        qh[a] = kq * ((g[a][1 + D] - eir * g[a][0]) * irs - vdv);
+                    }
                 }
 #pragma unroll
                 for (int a = 0; a < D; ++a) {
                     double F[Vc];
                     euler_flux<D>(u, q, a, F);
-                    if (VISC) ns_flux_sub<D>(q, g, dv, divv, a, p.gamma, p.nu, p.chi, F);
+                    if (VISC) {
+                        double ev = qh[a];
+#pragma unroll
+                        for (int b = 0; b < D; ++b) {
+                            F[1 + b] -= Pi[a][b];
+                            ev = fma(q.v[b], Pi[a][b], ev);
+                        }
+                        F[1 + D] -= ev;
+                    }
                     if (AV) {
 #pragma unroll
-                        for (int v = 0; v < Vc; ++v) F[v] -= eps * g[a][v];
+                        for (int v = 0; v < Vc; ++v) F[v] = fma(-epss, g[a][v], F[v]);
                     }
 #pragma unroll
                     for (int v = 0; v < Vc; ++v) GR[L::at2(a * Vc + v, j) * C + cl] = F[v];
@@ -284,9 +305,7 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
                 tile_load<M, C, L>(GR, (0 * Vc + v) * NTILE + jz, cl, n);
                 tile_x<DG_SEL_S, M>(n);
                 tile_load<M, C, L>(GR, (1 * Vc + v) * NTILE + jz, cl, b);
-                tile_y<DG_SEL_S, M>(b);
-#pragma unroll
-                for (int q = 0; q < MM; ++q) n[q] += b[q];
+                tile_y_acc<DG_SEL_S, M>(b, n);
                 if (D == 3) {
 #pragma unroll
                     for (int kk = 0; kk < NTILE; ++kk) {

@@ -29,6 +29,9 @@
 #define DG_SEL_S 2
 #define DG_SEL_VTG 3
 
+#ifndef DG_USE_DMMA
+#define DG_USE_DMMA 0
+#endif
 #ifndef DG_EVEN_ODD
 #define DG_EVEN_ODD 1
 #endif
@@ -239,6 +242,55 @@ __device__ __forceinline__ int pencil_base(int pen) {
     return (pen / STRIDE) * (STRIDE * M) + (pen % STRIDE);
 }
 
+// ---- fp64 tensor-core form of a sweep for m = 8 (experiment, DG_USE_DMMA; see profiles/r2_dmma.md) ----
+// One mma.sync.m8n8k4.f64 pair computes  D[j][n] = sum_i MAT[j][i] * X[i][n]  for 8 pencils n at once (K = 8 as two
+// k = 4 steps).  Fragments (PTX ISA, m8n8k4 .f64): A row-major, lane l holds A[l/4][l%4]; B, lane l holds B[l%4][l/4];
+// C/D, lane l holds D[l/4][2(l%4)] and D[l/4][2(l%4)+1].  Columns enumerate (pencil, cell) pairs, cell fastest.
+__device__ __forceinline__ void dmma884(double &d0, double &d1, double a, double b, double c0, double c1) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%4,%5};"
+                 : "=d"(d0), "=d"(d1)
+                 : "d"(a), "d"(b), "d"(c0), "d"(c1));
+}
+template <int SEL, int NPTS, int STRIDE, int C, int NT, int NSUM, bool ADD, bool SCALE, class L>
+__device__ __forceinline__ void sweep_dmma8(const double *src, int s0, int sum_slots, double *dst, int d0, int nslots,
+                                            double scale, int tid) {
+    constexpr int M = 8, NPEN = NPTS / M;
+    const int lane = tid & 31, warp = tid >> 5;
+    const int k = lane & 3, n = lane >> 2;
+    const double a0 = mat<SEL>(n * 8 + k), a1 = mat<SEL>(n * 8 + k + 4);
+    const int groups = nslots * NPEN * C / 8;            // NPEN * C is a multiple of 8 for m = 8
+    for (int grp = warp; grp < groups; grp += NT / 32) {
+        // operand B: element (k, k+4) of column n
+        const int pc = grp * 8 + n;
+        const int r = pc / C, cell = pc % C;
+        const int slot = r / NPEN, pb = pencil_base<M, STRIDE>(r % NPEN);
+        double b0 = src[L::at2(s0 + slot, pb + k * STRIDE) * C + cell];
+        double b1 = src[L::at2(s0 + slot, pb + (k + 4) * STRIDE) * C + cell];
+#pragma unroll
+        for (int q = 1; q < NSUM; ++q) {
+            b0 += src[L::at2(s0 + q * sum_slots + slot, pb + k * STRIDE) * C + cell];
+            b1 += src[L::at2(s0 + q * sum_slots + slot, pb + (k + 4) * STRIDE) * C + cell];
+        }
+        double e0, e1;
+        dmma884(e0, e1, a0, b0, 0.0, 0.0);
+        dmma884(e0, e1, a1, b1, e0, e1);
+        // result: row j = n, columns 2k and 2k+1
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+            const int pc2 = grp * 8 + 2 * k + e;
+            const int r2 = pc2 / C, cell2 = pc2 % C;
+            const int slot2 = r2 / NPEN, pb2 = pencil_base<M, STRIDE>(r2 % NPEN);
+            double val = e ? e1 : e0;
+            if (SCALE) val *= scale;
+            double *d = dst + L::at2(d0 + slot2, pb2 + n * STRIDE) * C + cell2;
+            if (ADD)
+                *d += val;
+            else
+                *d = val;
+        }
+    }
+}
+
 // Apply one 1D matrix along one axis to `nslots` arrays of NPTS points (slots s0 .. s0+nslots of src, d0 .. of dst):
 //   dst[d0+slot][p] (+)= scale * sum_i MAT[j][i] * (sum_{k<NSUM} src[s0 + k*sum_slots + slot][p_i])
 // src == dst (in place) is allowed: a thread owns whole pencils.
@@ -247,6 +299,11 @@ __device__ __forceinline__ void sweep(const double *src, int s0, int sum_slots, 
                                       double scale, int tid) {
     constexpr int NPEN = NPTS / M;
     static_assert(NT % C == 0, "threads per block must be a multiple of cells per block");
+    if (DG_USE_DMMA && M == 8 && (NPEN * C) % 8 == 0) {
+        // in-place sweeps are safe: a warp reads all 8 pencils of a group before it writes them, and groups are disjoint
+        sweep_dmma8<SEL, NPTS, STRIDE, C, NT, NSUM, ADD, SCALE, L>(src, s0, sum_slots, dst, d0, nslots, scale, tid);
+        return;
+    }
     const int cell = tid % C;
     const int total = nslots * NPEN;
     for (int r = tid / C; r < total; r += NT / C) {
@@ -973,8 +1030,9 @@ __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(co
     double *bar = sens + (AV ? 4 * (NT / 32) * C : 0);   // mbarrier of the bulk copies
     const int tid = threadIdx.x;
     const int cell0 = blockIdx.x * C;
-    // own modes of a full tile travel global -> RA as bulk asynchronous copies (one request per row segment)
-    const bool bulk = bulk_ok<C>(cell0, p.ncells);
+    // own modes of a full tile travel global -> RA as bulk asynchronous copies (one request per row segment);
+    // with fewer than 8 cells per block (16/32-byte segments, m >= 6) batched plain loads are cheaper here
+    const bool bulk = (C >= 8) && bulk_ok<C>(cell0, p.ncells);
     if (bulk) {
         if (tid == 0) mbar_init(bar, 1);
         __syncthreads();

@@ -39,6 +39,12 @@
 #ifndef DG_STAGE_NT
 #define DG_STAGE_NT 512
 #endif
+#ifndef DG_STAGE_NT_BIG
+#define DG_STAGE_NT_BIG 768
+#endif
+#ifndef DG_FACE_NT_BIG
+#define DG_FACE_NT_BIG 512
+#endif
 #ifndef DG_STAGE_MINB
 #define DG_STAGE_MINB 1
 #endif
@@ -77,7 +83,9 @@ struct Cfg {
     static constexpr int NQ = NQE + (GRAD ? (D - 1) * Vc : 0);
     static constexpr int RX = D * Vc * Np;                         // gradients -> fluxes (in place)
     static constexpr int FP = 2 * V * Np + RX;                     // doubles per cell
-    static constexpr int NT = DG_STAGE_NT;
+    // pencil-sweep configurations (3D, m >= 6: 2-4 cells per block): more warps hide the latency of the short row
+    // segments (measured at m = 8: 768 threads -13 % against 512)
+    static constexpr int NT = (D == 3 && M >= 6) ? DG_STAGE_NT_BIG : DG_STAGE_NT;
     // W^K per cell, wave-speed reduction scratch, partial sensor sums, one mbarrier
     static constexpr int extra_doubles(int c) { return c + 2 * (NT / 32) + (AV ? 4 * (NT / 32) * c : 0) + 2; }
     static constexpr int pick_c() {
@@ -730,13 +738,14 @@ __device__ __forceinline__ void load_own_modes(const double *__restrict__ w, int
 template <int D, int M, bool VISC, bool AV>
 struct FaceCfg {
     using K = Cfg<D, M, VISC, AV>;
-    static constexpr int NT = DG_FACE_NT;
+    static constexpr int BIG = (D == 3 && M >= 6);     // one large block per SM (measured at m = 8: -25 %)
+    static constexpr int NT = BIG ? DG_FACE_NT_BIG : DG_FACE_NT;
     // DIRECT (3D register-tile configurations): F1 reads the own modes straight from global memory / L1 like the
     // neighbour's (each is used once per axis), so no copy of the tile is staged in shared memory, the block does
     // not wait for it before the first axis, and only the face scratch remains (more cells or blocks per SM)
     static constexpr bool DIRECT = DG_FACE_DIRECT && K::BLK && (D == 3);
     static constexpr int FP = (DIRECT ? 0 : K::V * K::Np) + K::NQ * K::Nf;   // doubles per cell: [own modes +] one face
-    static constexpr int MINB = DIRECT ? DG_FACE_DIRECT_MINB : DG_FACE_MINB;   // resident blocks per SM (register cap)
+    static constexpr int MINB = DIRECT ? DG_FACE_DIRECT_MINB : (BIG ? 1 : DG_FACE_MINB);   // resident blocks per SM (register cap)
     static constexpr int CMAX = DIRECT ? 16 : 32;
     static constexpr int pick_c() {
         int c = CMAX;
@@ -978,7 +987,7 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA
 }
 
 template <int D, int M, bool VISC, bool AV>
-__global__ void __launch_bounds__(DG_FACE_NT, (FaceCfg<D, M, VISC, AV>::MINB)) dg_face_kernel(const DgStageArgs p) {
+__global__ void __launch_bounds__((FaceCfg<D, M, VISC, AV>::NT), (FaceCfg<D, M, VISC, AV>::MINB)) dg_face_kernel(const DgStageArgs p) {
     using K = Cfg<D, M, VISC, AV>;
     using FK = FaceCfg<D, M, VISC, AV>;
     constexpr int C = FK::C, NT = FK::NT, V = K::V, Np = K::Np;
@@ -1014,7 +1023,7 @@ __global__ void __launch_bounds__(DG_FACE_NT, (FaceCfg<D, M, VISC, AV>::MINB)) d
 // the stage kernel
 // ---------------------------------------------------------------------------------------------------
 template <int D, int M, bool VISC, bool AV>
-__global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(const DgStageArgs p) {
+__global__ void __launch_bounds__((Cfg<D, M, VISC, AV>::NT), DG_STAGE_MINB) dg_stage_kernel(const DgStageArgs p) {
     using K = Cfg<D, M, VISC, AV>;
     constexpr int C = K::C, NT = K::NT, V = K::V, Vc = K::Vc, Np = K::Np;
     constexpr bool GRAD = K::GRAD, BLK = K::BLK;
@@ -1387,7 +1396,7 @@ __global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_stage_kernel(co
 
 // standalone wave-speed kernel (after dg_set_state): load -> expand -> max
 template <int D, int M, bool VISC, bool AV>
-__global__ void __launch_bounds__(DG_STAGE_NT, DG_STAGE_MINB) dg_wavespeed_kernel(const DgStageArgs p) {
+__global__ void __launch_bounds__((Cfg<D, M, VISC, AV>::NT), DG_STAGE_MINB) dg_wavespeed_kernel(const DgStageArgs p) {
     using K = Cfg<D, M, VISC, AV>;
     constexpr int C = K::C, NT = K::NT, V = K::V, Vc = K::Vc, Np = K::Np;
     using L = Lay<M * M, Np, use_swizzle(M, C), use_rot(M, C, K::BLK)>;

@@ -171,7 +171,7 @@ def run_gpu(args):
     wk.initial_modes_slabbed(wl, out=host_in.numpy())
     t_ic = time.time() - t0
 
-    solver = dg.from_workload(wl)
+    solver = dg.from_workload(wl, **({"limiter_enable": 1} if args.limiter else {}))
     stream = torch.cuda.current_stream(dev)
     solver.set_state(host_in)
     info = solver.kernel_info()
@@ -269,7 +269,8 @@ def run_gpu(args):
         "warmup": args.warmup, "ms_per_step": t_max / args.steps * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": label, "cells": wl.ncells, "modes_per_cell": wl.modes, "variables": wl.nvar,
-                   "rk_stages": 3, "physics": ("NS" if wl.nu > 0 else "Euler") + ("+AV" if wl.av else ""),
+                   "rk_stages": 3, "physics": ("NS" if wl.nu > 0 else "Euler") + ("+AV" if wl.av else "") + (
+                       "+positivity limiter" if args.limiter else ""),
                    "replicas": world, "l2": "state %.2f GiB per buffer >> 126 MB L2 (no flush needed)" % (
                        wl.nvar * wl.modes * wl.ncells * 8 / 2 ** 30) if wl.nvar * wl.modes * wl.ncells * 8 > 4e8
                    else "state fits L2: L2-resident by design (reported as such)",
@@ -336,6 +337,8 @@ def main():
     ap.add_argument("--degree", type=int, default=None)
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--limiter", action="store_true",
+                    help="positivity limiter on (with cfg4: the paper's timing workload NS + AV + limiter, PAPER.md:800)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
     args.steps = max(args.steps, 1)

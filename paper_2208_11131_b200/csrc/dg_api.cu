@@ -30,7 +30,7 @@ int fail(int code, const char *fmt, const char *detail = "") {
 
 typedef cudaError_t (*launch_fn)(int, int, const DgStageArgs *, cudaStream_t, int);
 typedef cudaError_t (*upload_fn)(const DgTables *);
-typedef void (*info_fn)(int, int, int *, int *, int *);
+typedef void (*info_fn)(int, int, int *, int *, int *, int *);
 typedef cudaError_t (*config_fn)(int, int);
 typedef cudaError_t (*limit_fn)(double *, int, int, double, int *, cudaStream_t);
 
@@ -142,6 +142,7 @@ struct dg_solver {
     long long launches;
     long long steps;        // full RK steps since dg_set_state
     int kC, kNT, kSmem;
+    int fused_limiter;      // the stage kernel of this configuration applies the positivity limiter itself
 };
 
 namespace {
@@ -239,14 +240,14 @@ int enqueue_wavespeed(dg_solver *s) {
 
 // positivity limiter on a stage output (optional).  Nothing to limit for degree 0.
 int enqueue_limiter(dg_solver *s, double *w) {
-    if (!s->opt.limiter_enable || s->order < 2) return DG_OK;
+    if (!s->opt.limiter_enable || s->order < 2 || s->fused_limiter) return DG_OK;
     CU(s->fn.limit(w, s->V, s->ncells, s->gamma, s->flag, s->stream));
     return DG_OK;
 }
 
 // with the limiter on, the wave speeds of the new state (Eq. 23) are taken after it, by the stand-alone kernel
 int enqueue_post_step(dg_solver *s) {
-    if (!s->opt.limiter_enable || s->order < 2) return DG_OK;
+    if (!s->opt.limiter_enable || s->order < 2 || s->fused_limiter) return DG_OK;
     DgStageArgs a;
     fill_args(s, &a);
     a.w_prev = s->W0;
@@ -256,7 +257,10 @@ int enqueue_post_step(dg_solver *s) {
 
 // enqueue one full SSP-RK step (Shu-Osher forms)
 int enqueue_step(dg_solver *s) {
-    const bool lim = s->opt.limiter_enable && s->order >= 2;
+    // limiter as separate launches (+ a stand-alone wave-speed pass); register-tile configurations fuse both into
+    // the stage kernel instead (DgStageArgs::limiter)
+    const bool lim = s->opt.limiter_enable && s->order >= 2 && !s->fused_limiter;
+    const int fl = (s->opt.limiter_enable && s->order >= 2 && s->fused_limiter) ? 1 : 0;
     const int S = s->opt.rk_stages;
     dg_dt_kernel<<<1, 1, 0, s->stream>>>(s->scal, s->maxbits, s->opt.f_cfl, s->h, s->order, s->opt.fixed_dt);
     CU(cudaGetLastError());
@@ -289,6 +293,7 @@ int enqueue_step(dg_solver *s) {
             g.do_sensor = (i == 0) && s->av;
             g.commit_sensor = (i == 4) && s->av;
             g.do_wavespeed = (i == 4) && !lim;
+            g.limiter = fl;
             CU(s->fn.launch(s->visc, s->av, &g, s->stream, 0));
             int rc = enqueue_limiter(s, out[i]);
             if (rc) return rc;
@@ -313,6 +318,7 @@ int enqueue_step(dg_solver *s) {
         a.do_sensor = (i == 0) && s->av;
         a.commit_sensor = (i == S - 1) && s->av;
         a.do_wavespeed = (i == S - 1) && !lim;
+        a.limiter = fl;
         CU(s->fn.launch(s->visc, s->av, &a, s->stream, 0));
         int rc = enqueue_limiter(s, out);
         if (rc) return rc;
@@ -413,7 +419,7 @@ int init_common(dg_solver **out, const dg_mesh *mesh, int order, double gamma, d
         delete s;
         return fail(DG_ECUDA, "kernel configuration failed (needs an sm_100a device): %s", cudaGetErrorString(e));
     }
-    s->fn.info(s->visc, s->av, &s->kC, &s->kNT, &s->kSmem);
+    s->fn.info(s->visc, s->av, &s->kC, &s->kNT, &s->kSmem, &s->fused_limiter);
     *out = s;
     return DG_OK;
 }
@@ -534,7 +540,7 @@ int dg_step_async(dg_solver *s, int nsteps) {
         int rc = enqueue_wavespeed(s);
         if (rc) return rc;
     }
-    const bool lim = s->opt.limiter_enable && s->order >= 2;
+    const bool lim = s->opt.limiter_enable && s->order >= 2 && !s->fused_limiter;
     // dt kernel + (face, stage[, limiter]) per RK stage [+ wave-speed kernel]
     const int per_step = 1 + (2 + (lim ? 1 : 0)) * s->opt.rk_stages + (lim ? 1 : 0);
     if (s->opt.use_graph && nsteps > 0) {

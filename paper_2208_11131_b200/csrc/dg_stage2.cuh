@@ -17,6 +17,7 @@
 #pragma once
 
 #include "dg_stage.cuh"
+#include "dg_limiter.cuh"
 
 #ifndef DG_S2_NT3
 #define DG_S2_NT3 512
@@ -47,7 +48,11 @@ struct Cfg2 {
     // doubles per cell: U (nodal values) + GR (gradients -> fluxes)
     static constexpr int FP = V * Np + D * Vc * Np;
     // Wk[c], wave-speed scratch, sensor partials, S table
-    static constexpr int extra_doubles(int c) { return c + 2 * (NT / 32) + (AV ? 4 * (NT / 32) * c : 0) + M * M + 2; }
+    // ... and the positivity limiter's per-cell scratch (fused form, see the kernel's tail)
+    static constexpr int lim_doubles(int c) { return (D + 2 + 3) * c + c + (c + 1) / 2 + 2 + (D + 2) * c; }
+    static constexpr int extra_doubles(int c) {
+        return c + 2 * (NT / 32) + (AV ? 4 * (NT / 32) * c : 0) + M * M + 2 + lim_doubles(c);
+    }
     static constexpr int pick_c() {
         int c = CMAX;
         while (c > 1 && (c * FP + extra_doubles(c)) * 8 > (227 * 1024) / DG_S2_MINB - 1024) c >>= 1;
@@ -78,7 +83,11 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
     double *red = Wk + C;
     double *sens = red + 2 * (NT / 32);           // [4][NT/32][C] partial sensor sums (AV only)
     double *sS = sens + (AV ? 4 * (NT / 32) * C : 0);   // weak-derivative matrix S for run-time row indices
+    double *limsc = sS + M * M + 2;                     // limiter scratch (fused form)
+    double *ldev = limsc + LimScratch<D, C>::kDoubles;  // [Vc][C] sum_{l>0} |w_l| max|phi_l| of the new state
+    const bool lim = (p.limiter != 0);
     const int tid = threadIdx.x;
+    if (lim && tid < Vc * C) ldev[tid] = 0.0;
     const int cl = tid % C;
     const double ih = 1.0 / p.h;
     const double pref = (D == 3 ? 0.25 : 0.5) * ih;
@@ -340,6 +349,7 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
                 const double *bp = p.w_prev + (size_t)v * p.ncells + cg;
                 double *bo = p.w_out + (size_t)v * p.ncells + cg;
                 double wn[MM], wp[MM];
+                double gdev = 0.0;
 #pragma unroll
                 for (int q = 0; q < MM; ++q) {
                     wn[q] = need_n ? *row_ptr(bn, q * V, p.ncells) : 0.0;
@@ -366,8 +376,12 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
                         }
                     }
                     n[q] = wnew;
+                    if (lim && v < Vc && q != 0) gdev = fma(fabs(wnew), c_tab.Pend[1][q % M] * c_tab.Pend[1][q / M], gdev);
                 }
-                if (p.do_wavespeed && v < Vc) {
+                if (lim && v < Vc) {
+                    atomicAdd(&ldev[v * C + cl], gdev);
+                    tile_store<M, C, L>(U, g, cl, n);         // new modes: the limiter expands them itself
+                } else if (p.do_wavespeed && v < Vc) {
                     tile_x<DG_SEL_V, M>(n);
                     tile_y<DG_SEL_V, M>(n);
                     tile_store<M, C, L>(U, g, cl, n);
@@ -414,6 +428,8 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
                 for (int j = 0; j < M; ++j) in[j] = U[L::at2(v, q + j * MM) * C + cl];
                 const bool topxy = (q % M == M - 1) || (q / M == M - 1);
                 const int lxy = q % M + q / M;
+                const double bq = c_tab.Pend[1][q % M] * c_tab.Pend[1][q / M];   // max |P_lx P_ly| on the cell
+                double hdev = 0.0;
                 double pz[M];
                 apply1d<DG_SEL_VTG, M>(in, pz);
 #pragma unroll
@@ -445,8 +461,10 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
                             dA = fma(hwn[k][l], Ld, dA);
                         }
                     }
-                    if (p.do_wavespeed) U[L::at2(v, q + l * MM) * C + cl] = wnew;
+                    if (p.do_wavespeed || lim) U[L::at2(v, q + l * MM) * C + cl] = wnew;
+                    if (lim && v < Vc && (q + l) != 0) hdev = fma(fabs(wnew), bq * c_tab.Pend[1][l], hdev);
                 }
+                if (lim && v < Vc) atomicAdd(&ldev[v * C + cl], hdev);
             }
         }
         if (AV && p.do_sensor) {
@@ -481,8 +499,78 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
             p.sens_prev[c] = p.sens_new[c];
             p.sens_prev[p.ncells + c] = p.sens_new[p.ncells + c];
         }
-        // ---- wave speeds of the new state for the next step's Eq. 23 ----
-        if (p.do_wavespeed) {
+        if (lim) {
+            // ---- positivity limiter on the stage output (Eq. 47; readings L1-L6), fused: the new
+            //      modes of the d+2 conserved fields are still in U, the face point values go to the (now free) flux
+            //      array; cells with F != 1 re-read their freshly written rows (L2) and scale every mode but the mean ----
+            //      Shortcut that cannot change the result: |phi_l| <= prod_a sqrt(2 l_a + 1) on the whole cell, so
+            //      rho >= rho_bar - dev_rho, |m_b| <= |m_bar_b| + dev_b, e >= e_bar - dev_e at every evaluation point;
+            //      if these bounds already keep rho and p above their floors (with a factor 2 of margin) in all cells
+            //      of the block, F = 1 exactly as the full evaluation would find, and the evaluation is skipped.
+            __syncthreads();
+            int full = 0;
+            if (tid < C && cell0 + tid < p.ncells) {
+                double mb[Vc], dv_[Vc];
+#pragma unroll
+                for (int v = 0; v < Vc; ++v) {
+                    mb[v] = U[L::at2(v, 0) * C + tid];
+                    dv_[v] = ldev[v * C + tid];
+                }
+                double mm = 0.0, mh = 0.0;
+#pragma unroll
+                for (int b = 0; b < D; ++b) {
+                    mm = fma(mb[1 + b], mb[1 + b], mm);
+                    const double hi = fabs(mb[1 + b]) + dv_[1 + b];
+                    mh = fma(hi, hi, mh);
+                }
+                const double pbar = (p.gamma - 1.0) * (mb[1 + D] - 0.5 * mm / mb[0]);
+                const double rlo = mb[0] - dv_[0];
+                const double plo = (p.gamma - 1.0) * ((mb[1 + D] - dv_[1 + D]) - 0.5 * mh / rlo);
+                const bool safe = (mb[0] > 0.0) && (pbar > 0.0) && (rlo > 2.0e-6 * mb[0]) && (plo > 2.0e-6 * pbar);
+                full = safe ? 0 : 1;
+            }
+            full = __syncthreads_or(full);
+            const LimScratch<D, C> sc(limsc);
+            if (full) limiter_core<D, M, C, NT, true, L>(U, GR, sc, p.gamma, p.flag, cell0, p.ncells, tid);
+            const double F = full ? sc.Fc[cl] : 1.0;
+            if (F != 1.0 && active) {
+                for (int r = tid / C; r < Vc * Np; r += NT / C) {
+                    const int v = r % Vc, mode = r / Vc;
+                    if (mode == 0) continue;
+                    double *q = p.w_out + (size_t)(mode * V + v) * p.ncells + cg;
+                    *q = F * __ldcg(q);
+                }
+            }
+            // wave speeds of the limited state (reading L6): u(x) = u_bar + F (u(x) - u_bar) at the volume points
+            if (p.do_wavespeed && !full) {
+                expand_volume<D, M, C, NT, true, L>(U, Vc, tid);
+                wavespeed_points<D, M, C, NT, L>(U, p.gamma, p.flag, red, p.maxbits, tid);
+            } else if (p.do_wavespeed) {
+                double cmax = 0.0, vmax = 0.0;
+                bool bad = false;
+                for (int it = tid; it < Np * C; it += NT) {
+                    const int j = it / C;
+                    double u[Vc];
+#pragma unroll
+                    for (int v = 0; v < Vc; ++v) {
+                        const double x = U[L::at2(v, j) * C + cl], mv = sc.mean[v * C + cl];
+                        u[v] = (F == 1.0) ? x : fma(F, x - mv, mv);
+                    }
+                    const Prim<D> q = primitives<D>(u, p.gamma);
+                    bad |= !(q.rho > 0.0) || !(q.p > 0.0);
+                    double v2 = 0.0;
+#pragma unroll
+                    for (int b = 0; b < D; ++b) v2 = fma(q.v[b], q.v[b], v2);
+                    const double cs = fast_sqrt(p.gamma * q.p * q.ir);
+                    const double vm = fast_sqrt(v2);
+                    cmax = (cs > cmax) ? cs : cmax;
+                    vmax = (vm > vmax) ? vm : vmax;
+                }
+                if (bad) atomicOr(p.flag, 4);
+                block_max2<NT>(cmax, vmax, red, p.maxbits, tid);
+            }
+        } else if (p.do_wavespeed) {
+            // ---- wave speeds of the new state for the next step's Eq. 23 ----
             __syncthreads();
             if (D == 3) expand_volume<D, M, C, NT, true, L>(U, Vc, tid);
             wavespeed_points<D, M, C, NT, L>(U, p.gamma, p.flag, red, p.maxbits, tid);

@@ -20,5 +20,6 @@ struct DgStageArgs {
     double rk_a, rk_b, rk_c;  // u^(i) = rk_a u^n + rk_b u^(i-1) + rk_c dt L(u^(i-1))
     double aux_a, aux_b, aux_c;
     int do_sensor, do_wavespeed, commit_sensor, rhs_only;
+    int limiter;              // 1: positivity limiter on the stage output inside the stage kernel (dg_stage2_kernel only)
     int total_degree;         // 1: modes with sum_a l_a > n are discarded: their rows stay zero
 };

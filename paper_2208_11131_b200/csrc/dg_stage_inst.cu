@@ -3,7 +3,6 @@
 // with -DDG_DIM=2|3 -DDG_M=1..8 (keeps ptxas work parallel and each image small).
 #include "dg_stage.cuh"
 #include "dg_stage2.cuh"
-#include "dg_limiter.cuh"
 #include "dg_dispatch.h"
 
 #ifndef DG_DIM
@@ -74,7 +73,8 @@ cudaError_t launch(const DgStageArgs &a, cudaStream_t st, int wavespeed_only) {
 }
 
 template <bool VISC, bool AV>
-void info(int *c, int *nt, int *smem) {
+void info(int *c, int *nt, int *smem, int *fused_limiter) {
+    *fused_limiter = dgk::Cfg<DG_DIM, DG_M, VISC, AV>::PP ? 1 : 0;
     using K = dgk::Cfg<DG_DIM, DG_M, VISC, AV>;
     if constexpr (K::PP) {
         using K2 = dgk::Cfg2<DG_DIM, DG_M, VISC, AV>;
@@ -110,11 +110,11 @@ cudaError_t DG_FN(dg_upload, DG_DIM, DG_M)(const DgTables *t) {
     return cudaMemcpyToSymbol(c_tab, t, sizeof(DgTables));
 }
 
-void DG_FN(dg_info, DG_DIM, DG_M)(int visc, int av, int *c, int *nt, int *smem) {
-    if (visc && av) return info<true, true>(c, nt, smem);
-    if (visc) return info<true, false>(c, nt, smem);
-    if (av) return info<false, true>(c, nt, smem);
-    return info<false, false>(c, nt, smem);
+void DG_FN(dg_info, DG_DIM, DG_M)(int visc, int av, int *c, int *nt, int *smem, int *fused_limiter) {
+    if (visc && av) return info<true, true>(c, nt, smem, fused_limiter);
+    if (visc) return info<true, false>(c, nt, smem, fused_limiter);
+    if (av) return info<false, true>(c, nt, smem, fused_limiter);
+    return info<false, false>(c, nt, smem, fused_limiter);
 }
 
 cudaError_t DG_FN(dg_config, DG_DIM, DG_M)(int visc, int av) {

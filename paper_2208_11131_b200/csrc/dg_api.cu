@@ -30,7 +30,7 @@ int fail(int code, const char *fmt, const char *detail = "") {
 
 typedef cudaError_t (*launch_fn)(int, int, const DgStageArgs *, cudaStream_t, int);
 typedef cudaError_t (*upload_fn)(const DgTables *);
-typedef void (*info_fn)(int, int, int *, int *, int *, int *);
+typedef void (*info_fn)(int, int, int *, int *, int *, int *, int *);
 typedef cudaError_t (*config_fn)(int, int);
 typedef cudaError_t (*limit_fn)(double *, int, int, double, int *, cudaStream_t);
 
@@ -62,14 +62,37 @@ __global__ void dg_dt_kernel(double *scal, unsigned long long *maxbits, double f
     maxbits[1] = 0ull;
 }
 
+// element (row, cell) of an internal array of R rows: structure of arrays (B = 0) or B-cell blocks (GLay in dg_stage.cuh)
+__host__ __device__ inline size_t gidx(size_t row, int cell, int ncells, int B, size_t R) {
+    return B ? ((size_t)(cell / B) * R + row) * B + cell % B : row * (size_t)ncells + cell;
+}
+
+// boundary conversion for the block layout: ext[(mode*nv + v)*ncells + cell] <-> internal row mode*V + var0 + v
+__global__ void dg_pack_kernel(double *w, const double *ext, int V, int var0, int nv, int nmodes, int ncells, int B) {
+    const size_t total = (size_t)nmodes * nv * ncells;
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+        const int cell = (int)(i % ncells);
+        const int r = (int)(i / ncells);
+        w[gidx((size_t)(r / nv) * V + var0 + r % nv, cell, ncells, B, (size_t)V * nmodes)] = ext[i];
+    }
+}
+__global__ void dg_unpack_kernel(double *ext, const double *w, int V, int var0, int nv, int nmodes, int ncells, int B) {
+    const size_t total = (size_t)nmodes * nv * ncells;
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+        const int cell = (int)(i % ncells);
+        const int r = (int)(i / ncells);
+        ext[i] = w[gidx((size_t)(r / nv) * V + var0 + r % nv, cell, ncells, B, (size_t)V * nmodes)];
+    }
+}
+
 // |K| sum_cells w_0 per conserved variable: one block per variable, fixed-shape compensated reduction.
-__global__ void __launch_bounds__(1024) dg_totals_kernel(const double *w, int V, int ncells, double vol, double *out) {
+__global__ void __launch_bounds__(1024) dg_totals_kernel(const double *w, int V, int ncells, double vol, double *out,
+                                                        int B, size_t R) {
     __shared__ double ss[1024], sc[1024];
     const int v = blockIdx.x;
-    const double *row = w + (size_t)v * ncells;   // mode 0, variable v
-    double s = 0.0, c = 0.0;                      // Neumaier summation
+    double s = 0.0, c = 0.0;                      // Neumaier summation over row v (mode 0, variable v)
     for (int i = threadIdx.x; i < ncells; i += 1024) {
-        const double x = row[i];
+        const double x = w[gidx((size_t)v, i, ncells, B, R)];
         const double t = s + x;
         c += (fabs(s) >= fabs(x)) ? ((s - t) + x) : ((x - t) + s);
         s = t;
@@ -91,7 +114,8 @@ __global__ void __launch_bounds__(1024) dg_totals_kernel(const double *w, int V,
 }
 
 // total-degree basis: zero the rows of the discarded modes (sum_a l_a > n) of `nv` variables
-__global__ void dg_mask_modes_kernel(double *w, int pitch_vars, int var0, int nv, int nmodes, int m, int dim, int ncells) {
+__global__ void dg_mask_modes_kernel(double *w, int pitch_vars, int var0, int nv, int nmodes, int m, int dim, int ncells,
+                                     int B) {
     const size_t total = (size_t)nmodes * nv * ncells;
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
         const int cell = (int)(i % ncells);
@@ -102,7 +126,7 @@ __global__ void dg_mask_modes_kernel(double *w, int pitch_vars, int var0, int nv
             lsum += rem % m;
             rem /= m;
         }
-        if (lsum > m - 1) w[((size_t)mode * pitch_vars + var0 + v) * ncells + cell] = 0.0;
+        if (lsum > m - 1) w[gidx((size_t)mode * pitch_vars + var0 + v, cell, ncells, B, (size_t)pitch_vars * nmodes)] = 0.0;
     }
 }
 
@@ -128,6 +152,10 @@ struct dg_solver {
     dg_options opt;
     int visc, av, Vc, V, M;
     size_t nstate;          // V * M * ncells doubles
+    int B;                  // cells per block of the internal layout (0: structure of arrays = the C-ABI layout)
+    int ncpad;              // ncells rounded up to a multiple of B
+    size_t nalloc;          // V * M * ncpad doubles per state buffer
+    double *xbuf;           // B > 0: staging buffer for the boundary conversion (nstate doubles)
     Dispatch fn;
     cudaStream_t stream;
     double *W0, *WA, *WB, *WC, *WD;   // u^n and stage buffers (WC, WD: five-stage scheme only)
@@ -156,13 +184,14 @@ size_t workspace_layout(dg_solver *s, char *base) {
         off += align_up(bytes, 256);
         return p;
     };
-    const size_t sb = s->nstate * sizeof(double);
+    const size_t sb = s->nalloc * sizeof(double);
     s->W0 = (double *)take(sb);
     s->WA = (double *)take(sb);
     s->WB = (s->opt.rk_stages >= 3) ? (double *)take(sb) : nullptr;
     s->WC = (s->opt.rk_stages == 5) ? (double *)take(sb) : nullptr;
     s->WD = (s->opt.rk_stages == 5) ? (double *)take(sb) : nullptr;
-    s->flux = (double *)take((size_t)s->dim * s->Vc * (s->M / s->order) * s->ncells * sizeof(double));
+    s->flux = (double *)take((size_t)s->dim * s->Vc * (s->M / s->order) * s->ncpad * sizeof(double));
+    s->xbuf = s->B ? (double *)take(s->nstate * sizeof(double)) : nullptr;
     s->scal = (double *)take(16 * sizeof(double));
     s->maxbits = (unsigned long long *)take(4 * sizeof(unsigned long long));
     s->flag = (int *)take(sizeof(int));
@@ -324,7 +353,7 @@ int enqueue_step(dg_solver *s) {
         if (rc) return rc;
         prev = out;
     }
-    if (S == 1) CU(cudaMemcpyAsync(s->W0, s->WA, s->nstate * sizeof(double), cudaMemcpyDeviceToDevice, s->stream));
+    if (S == 1) CU(cudaMemcpyAsync(s->W0, s->WA, s->nalloc * sizeof(double), cudaMemcpyDeviceToDevice, s->stream));
     return enqueue_post_step(s);
 }
 
@@ -378,6 +407,9 @@ int init_common(dg_solver **out, const dg_mesh *mesh, int order, double gamma, d
     for (int a = 0; a < s->dim; ++a) s->M *= order;
     s->nstate = (size_t)s->V * s->M * s->ncells;
     s->fn = kDispatch[s->dim - 2][order - 1];
+    s->fn.info(s->visc, s->av, &s->kC, &s->kNT, &s->kSmem, &s->fused_limiter, &s->B);
+    s->ncpad = s->B ? (s->ncells + s->B - 1) / s->B * s->B : s->ncells;
+    s->nalloc = (size_t)s->V * s->M * s->ncpad;
     const size_t need = workspace_layout(s, nullptr);
     if (need_only) {
         *need_only = need;
@@ -419,7 +451,7 @@ int init_common(dg_solver **out, const dg_mesh *mesh, int order, double gamma, d
         delete s;
         return fail(DG_ECUDA, "kernel configuration failed (needs an sm_100a device): %s", cudaGetErrorString(e));
     }
-    s->fn.info(s->visc, s->av, &s->kC, &s->kNT, &s->kSmem, &s->fused_limiter);
+    s->fn.info(s->visc, s->av, &s->kC, &s->kNT, &s->kSmem, &s->fused_limiter, &s->B);
     *out = s;
     return DG_OK;
 }
@@ -439,11 +471,30 @@ int zero_fill(dg_solver *s, double *dst, size_t count) {
     return DG_OK;
 }
 
-// copy between a caller buffer with `nv` variables per mode and the internal V-variable layout
-int copy_vars(dg_solver *s, void *dst, size_t dpitch_vars, const void *src, size_t spitch_vars, size_t nv) {
+// caller buffer ext[(mode*nv + v)*ncells + cell] (HOST or DEVICE) -> rows mode*V + var0 + v of the internal array W
+int to_internal(dg_solver *s, double *W, int var0, const double *ext, int nv) {
     const size_t row = (size_t)s->ncells * sizeof(double);
-    CU(cudaMemcpy2DAsync(dst, dpitch_vars * row, src, spitch_vars * row, nv * row, s->M, cudaMemcpyDefault,
-                         s->stream));
+    if (!s->B) {
+        CU(cudaMemcpy2DAsync(W + (size_t)var0 * s->ncells, (size_t)s->V * row, ext, (size_t)nv * row, (size_t)nv * row, s->M,
+                             cudaMemcpyDefault, s->stream));
+        return DG_OK;
+    }
+    CU(cudaMemcpyAsync(s->xbuf, ext, (size_t)s->M * nv * row, cudaMemcpyDefault, s->stream));
+    dg_pack_kernel<<<1024, 256, 0, s->stream>>>(W, s->xbuf, s->V, var0, nv, s->M, s->ncells, s->B);
+    CU(cudaGetLastError());
+    return DG_OK;
+}
+// and back
+int from_internal(dg_solver *s, double *ext, const double *W, int var0, int nv) {
+    const size_t row = (size_t)s->ncells * sizeof(double);
+    if (!s->B) {
+        CU(cudaMemcpy2DAsync(ext, (size_t)nv * row, W + (size_t)var0 * s->ncells, (size_t)s->V * row, (size_t)nv * row, s->M,
+                             cudaMemcpyDefault, s->stream));
+        return DG_OK;
+    }
+    dg_unpack_kernel<<<1024, 256, 0, s->stream>>>(s->xbuf, W, s->V, var0, nv, s->M, s->ncells, s->B);
+    CU(cudaGetLastError());
+    CU(cudaMemcpyAsync(ext, s->xbuf, (size_t)s->M * nv * row, cudaMemcpyDefault, s->stream));
     return DG_OK;
 }
 
@@ -498,11 +549,11 @@ int dg_set_stream(dg_solver *s, void *cuda_stream) {
 int dg_set_state(dg_solver *s, const double *w, size_t count) {
     if (!s || !w) return fail(DG_EINVAL, "NULL argument");
     if (count != (size_t)s->Vc * s->M * s->ncells) return fail(DG_EINVAL, "count must be Vc*M*Ncells");
-    CU(cudaMemsetAsync(s->W0, 0, s->nstate * sizeof(double), s->stream));
-    int rc = copy_vars(s, s->W0, s->V, w, s->Vc, s->Vc);
+    CU(cudaMemsetAsync(s->W0, 0, s->nalloc * sizeof(double), s->stream));
+    int rc = to_internal(s, s->W0, 0, w, s->Vc);
     if (rc) return rc;
     if (s->opt.basis) {     // L2 projection onto the kept (orthonormal) modes
-        dg_mask_modes_kernel<<<1024, 256, 0, s->stream>>>(s->W0, s->V, 0, s->Vc, s->M, s->order, s->dim, s->ncells);
+        dg_mask_modes_kernel<<<1024, 256, 0, s->stream>>>(s->W0, s->V, 0, s->Vc, s->M, s->order, s->dim, s->ncells, s->B);
         CU(cudaGetLastError());
     }
     if (s->av) {
@@ -523,10 +574,10 @@ int dg_set_alpha(dg_solver *s, const double *alpha, size_t count) {
     if (!s || !alpha) return fail(DG_EINVAL, "NULL argument");
     if (!s->av) return fail(DG_EINVAL, "artificial viscosity is not enabled");
     if (count != (size_t)s->M * s->ncells) return fail(DG_EINVAL, "count must be M*Ncells");
-    int rc = copy_vars(s, s->W0 + (size_t)s->Vc * s->ncells, s->V, alpha, 1, 1);
+    int rc = to_internal(s, s->W0, s->Vc, alpha, 1);
     if (rc) return rc;
     if (s->opt.basis) {
-        dg_mask_modes_kernel<<<1024, 256, 0, s->stream>>>(s->W0, s->V, s->Vc, 1, s->M, s->order, s->dim, s->ncells);
+        dg_mask_modes_kernel<<<1024, 256, 0, s->stream>>>(s->W0, s->V, s->Vc, 1, s->M, s->order, s->dim, s->ncells, s->B);
         CU(cudaGetLastError());
     }
     CU(cudaStreamSynchronize(s->stream));
@@ -598,7 +649,7 @@ int dg_step(dg_solver *s, int nsteps) {
 int dg_get_state(dg_solver *s, double *w, size_t count) {
     if (!s || !w) return fail(DG_EINVAL, "NULL argument");
     if (count != (size_t)s->Vc * s->M * s->ncells) return fail(DG_EINVAL, "count must be Vc*M*Ncells");
-    int rc = copy_vars(s, w, s->Vc, s->W0, s->V, s->Vc);
+    int rc = from_internal(s, w, s->W0, 0, s->Vc);
     if (rc) return rc;
     CU(cudaStreamSynchronize(s->stream));
     return DG_OK;
@@ -608,7 +659,7 @@ int dg_get_alpha(dg_solver *s, double *alpha, size_t count) {
     if (!s || !alpha) return fail(DG_EINVAL, "NULL argument");
     if (count != (size_t)s->M * s->ncells) return fail(DG_EINVAL, "count must be M*Ncells");
     if (!s->av) return zero_fill(s, alpha, count);
-    int rc = copy_vars(s, alpha, 1, s->W0 + (size_t)s->Vc * s->ncells, s->V, 1);
+    int rc = from_internal(s, alpha, s->W0, s->Vc, 1);
     if (rc) return rc;
     CU(cudaStreamSynchronize(s->stream));
     return DG_OK;
@@ -618,7 +669,7 @@ int dg_conserved_totals(dg_solver *s, double totals[5]) {
     if (!s || !totals) return fail(DG_EINVAL, "NULL argument");
     double vol = 1.0;
     for (int a = 0; a < s->dim; ++a) vol *= s->h;
-    dg_totals_kernel<<<s->Vc, 1024, 0, s->stream>>>(s->W0, s->V, s->ncells, vol, s->scal + 8);
+    dg_totals_kernel<<<s->Vc, 1024, 0, s->stream>>>(s->W0, s->V, s->ncells, vol, s->scal + 8, s->B, (size_t)s->V * s->M);
     CU(cudaGetLastError());
     s->launches += 1;
     double t[5] = {0, 0, 0, 0, 0};
@@ -640,11 +691,11 @@ int dg_eval_rhs(dg_solver *s, double *out, size_t count, double *alpha_out, size
     a.rhs_only = 1;
     CU(s->fn.launch(s->visc, s->av, &a, s->stream, 0));
     s->launches += 2;
-    int rc = copy_vars(s, out, s->Vc, s->WA, s->V, s->Vc);
+    int rc = from_internal(s, out, s->WA, 0, s->Vc);
     if (rc) return rc;
     if (alpha_out) {
         if (s->av) {
-            rc = copy_vars(s, alpha_out, 1, s->WA + (size_t)s->Vc * s->ncells, s->V, 1);
+            rc = from_internal(s, alpha_out, s->WA, s->Vc, 1);
             if (rc) return rc;
         } else {
             rc = zero_fill(s, alpha_out, alpha_count);
@@ -662,7 +713,7 @@ int dg_profile_stage(dg_solver *s, int reps, double *face_ms, double *stage_ms) 
     if (s->opt.rk_stages >= 3) {
         // the middle stage of SSP-RK3 with its real combine arguments (reads u^n and u^(i-1), writes u^(i)):
         // u^(i-1) := a copy of the current state in WA, output to WB; W0 (the state) is not modified
-        CU(cudaMemcpyAsync(s->WA, s->W0, s->nstate * sizeof(double), cudaMemcpyDeviceToDevice, s->stream));
+        CU(cudaMemcpyAsync(s->WA, s->W0, s->nalloc * sizeof(double), cudaMemcpyDeviceToDevice, s->stream));
         a.w_prev = s->WA;
         a.w_n = s->W0;
         a.w_out = s->WB;

@@ -13,7 +13,7 @@ struct DgTables;
     cudaError_t DG_FN(dg_launch, d, m)(int visc, int av, const DgStageArgs *a, cudaStream_t st,       \
                                        int wavespeed_only);                                            \
     cudaError_t DG_FN(dg_upload, d, m)(const DgTables *t);                                             \
-    void DG_FN(dg_info, d, m)(int visc, int av, int *c, int *nt, int *smem, int *fused_limiter);                           \
+    void DG_FN(dg_info, d, m)(int visc, int av, int *c, int *nt, int *smem, int *fused_limiter, int *bsz);                           \
     cudaError_t DG_FN(dg_config, d, m)(int visc, int av);                                              \
     cudaError_t DG_FN(dg_limit, d, m)(double *w, int V, int ncells, double gamma, int *flag, cudaStream_t st);
 

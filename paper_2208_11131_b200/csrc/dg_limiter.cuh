@@ -188,11 +188,13 @@ __global__ void __launch_bounds__(256, 2) dg_limiter_kernel(double *w, int V, in
     const int cl = tid % C, g = tid / C;
     constexpr int G = NT / C;
     const int cg = min(cell0 + cl, ncells - 1);
+    const unsigned grs = GLay<D, M>::rs(ncells);
+    double *wc = w + GLay<D, M>::cell(cg, V * Np);               // (row 0, this thread's cell), V variables per mode
 
     for (int mode = g; mode < Np; mode += G) {
 #pragma unroll
         for (int v = 0; v < Vc; ++v) {
-            const double x = w[(size_t)(mode * V + v) * ncells + cg]   /* rewritten below: no non-coherent load */;
+            const double x = wc[(size_t)(mode * V + v) * grs]   /* rewritten below: no non-coherent load */;
             RA[(v * Np + mode) * C + cl] = x;
             NV[(v * Np + mode) * C + cl] = x;
         }
@@ -207,7 +209,7 @@ __global__ void __launch_bounds__(256, 2) dg_limiter_kernel(double *w, int V, in
                 if (mode == 0) continue;
 #pragma unroll
                 for (int v = 0; v < Vc; ++v)
-                    w[(size_t)(mode * V + v) * ncells + cg] = F * RA[(v * Np + mode) * C + cl];
+                    wc[(size_t)(mode * V + v) * grs] = F * RA[(v * Np + mode) * C + cl];
             }
         }
     }

@@ -29,6 +29,9 @@
 #define DG_SEL_S 2
 #define DG_SEL_VTG 3
 
+#ifndef DG_AOSOA
+#define DG_AOSOA 1
+#endif
 #ifndef DG_USE_DMMA
 #define DG_USE_DMMA 0
 #endif
@@ -657,6 +660,23 @@ __device__ __forceinline__ double *row_ptr(double *base, unsigned row, unsigned 
     return base + (unsigned long long)row * ncells;
 }
 
+// Layout of the state and face-flux arrays in global memory.  Default (B = 0): structure of arrays,
+// a[row * ncells + cell], the layout of the C-ABI.  Pencil-sweep configurations in 3D (m >= 6) keep only B = 2 or 4
+// cells per block in shared memory, and a row segment of B * 8 bytes per request leaves the kernels waiting on
+// thousands of 16-byte sectors per tile (measured: 63 % of the m = 8 stage kernel, L2-resident or not).  They use
+// an array of B-cell blocks instead, a[((cell / B) * R + row) * B + cell % B] (R rows per array): the rows of a tile are
+// adjacent, every request is a full line.  dg_api.cu converts at the boundary (dg_pack_kernel / dg_unpack_kernel).
+template <int D, int M>
+struct GLay {
+    static constexpr int B = (DG_AOSOA && D == 3 && M >= 6) ? Cfg<D, M, true, true>::C : 0;
+    // offset of (row 0, cell c) in an array of R rows
+    static __host__ __device__ __forceinline__ size_t cell(int c, int R) {
+        return B ? ((size_t)(c / (B ? B : 1)) * R * B + c % (B ? B : 1)) : (size_t)c;
+    }
+    // distance between consecutive rows of one cell
+    static __host__ __device__ __forceinline__ unsigned rs(int ncells) { return B ? (unsigned)B : (unsigned)ncells; }
+};
+
 // ---- bulk asynchronous copies (TMA engine, 1D): global -> shared, completion on an mbarrier ----
 __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(void *bar, unsigned count) {
@@ -706,12 +726,14 @@ __device__ __forceinline__ bool bulk_ok(int cell0, int ncells) {
 // cell tid % C and the modes g, g+G, ... (g = tid / C, G = NT / C) of every variable; its loads are issued in
 // batches of up to 12 before the first store (one DRAM round trip per batch).
 template <int V, int Np, int C, int NT, class L>
-__device__ __forceinline__ void load_own_modes(const double *__restrict__ w, int ncells, int cg, double *RA, int tid) {
+__device__ __forceinline__ void load_own_modes(const double *__restrict__ wcell, unsigned rs, double *RA, int tid) {
+    // wcell = address of (row 0, this thread's cell), rs = row stride (GLay)
     constexpr int G = NT / C;
     constexpr int NK = (Np + G - 1) / G;
     constexpr int KB = (12 / V) < 1 ? 1 : (12 / V);          // k-steps per batch
+    const unsigned ncells = rs;
     const int cl = tid % C, g = tid / C;
-    const double *base = w + (size_t)(g * V) * ncells + cg;
+    const double *base = wcell + (size_t)(g * V) * rs;
 #pragma unroll
     for (int k0 = 0; k0 < NK; k0 += KB) {
         double t[KB][V];
@@ -783,6 +805,9 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA
         const int cell = tid % C;
         const int nc = nbr[A * C + cell];
         const int oc = min(cell0 + cell, p.ncells - 1);
+        using GL = GLay<D, M>;
+        const unsigned grs = GL::rs(p.ncells);
+        const double *wnb = p.w_prev + GL::cell(nc, V * K::Np), *wow = p.w_prev + GL::cell(oc, V * K::Np);
         // the upper x neighbour of every cell but the last one of the tile is the next cell of the tile itself
         const bool from_tile = !FK::DIRECT && (A == 0) && (cell < C - 1) && (cell0 + cell + 1 < p.ncells) &&
                                (nc == cell0 + cell + 1);
@@ -800,13 +825,11 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA
                         for (int l = 0; l < M; ++l) nb[kk][l] = RA[LV::at2(v, base + l * SA) * C + cell + 1];
                     } else {
 #pragma unroll
-                        for (int l = 0; l < M; ++l)
-                            nb[kk][l] = __ldg(p.w_prev + (size_t)((base + l * SA) * V + v) * p.ncells + nc);
+                        for (int l = 0; l < M; ++l) nb[kk][l] = __ldg(row_ptr(wnb, (base + l * SA) * V + v, grs));
                     }
                     if (FK::DIRECT) {
 #pragma unroll
-                        for (int l = 0; l < M; ++l)
-                            ow[kk][l] = __ldg(p.w_prev + (size_t)((base + l * SA) * V + v) * p.ncells + oc);
+                        for (int l = 0; l < M; ++l) ow[kk][l] = __ldg(row_ptr(wow, (base + l * SA) * V + v, grs));
                     }
                 }
             }
@@ -939,7 +962,10 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA
     __syncthreads();
 
     // F4: project the face flux on the transverse modes (g_k phi_l(xi_k) of Eq. 20's surface lines) -> global
-    double *out = p.flux + (size_t)A * Vc * Nf * p.ncells;
+    // flux array: D * Vc * Nf rows [axis][var][transverse index]
+    using GLF = GLay<D, M>;
+    const unsigned frs = GLF::rs(p.ncells);
+    double *out = p.flux + (size_t)A * Vc * Nf * frs;
     if (TILE) {
         for (int it = tid; it < Vc * C; it += NT) {
             const int cell = it % C, g = it / C;
@@ -949,7 +975,8 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA
             if (!K::PP || A >= 2) tile_y<DG_SEL_VTG, M>(t);
             if (cell0 + cell < p.ncells) {
 #pragma unroll
-                for (int q = 0; q < M * M; ++q) out[(size_t)(g * Nf + q) * p.ncells + cell0 + cell] = t[q];
+                for (int q = 0; q < M * M; ++q)
+                    out[(size_t)(g * Nf + q) * frs + GLF::cell(cell0 + cell, D * Vc * Nf)] = t[q];
             }
         }
     } else {
@@ -980,7 +1007,8 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA
                 res[0] = in[0] * (D == 3 ? 4.0 : 2.0);
             }
 #pragma unroll
-            for (int j = 0; j < M; ++j) out[(size_t)(off + j * STR) * p.ncells + cell0 + cell] = res[j];
+            for (int j = 0; j < M; ++j)
+                out[(size_t)(off + j * STR) * frs + GLF::cell(cell0 + cell, D * Vc * Nf)] = res[j];
         }
     }
     __syncthreads();
@@ -999,7 +1027,8 @@ __global__ void __launch_bounds__((FaceCfg<D, M, VISC, AV>::NT), (FaceCfg<D, M, 
     const int tid = threadIdx.x;
     const TilePos<D, C> pos(p, tid % C);
     const int cell0 = pos.cell0;
-    const bool bulk = !FK::DIRECT && bulk_ok<C>(cell0, p.ncells);
+    using GL = GLay<D, M>;
+    const bool bulk = !FK::DIRECT && GL::B == 0 && bulk_ok<C>(cell0, p.ncells);
     if (bulk) {
         if (tid == 0) mbar_init(bar, 1);
         __syncthreads();
@@ -1012,7 +1041,7 @@ __global__ void __launch_bounds__((FaceCfg<D, M, VISC, AV>::NT), (FaceCfg<D, M, 
     if (bulk)
         mbar_wait(bar, 0);
     else if (!FK::DIRECT)
-        load_own_modes<V, Np, C, NT, typename FK::LV>(p.w_prev, p.ncells, pos.cg, RA, tid);
+        load_own_modes<V, Np, C, NT, typename FK::LV>(p.w_prev + GL::cell(pos.cg, V * Np), GL::rs(p.ncells), RA, tid);
     __syncthreads();
     face_axis<D, M, VISC, AV, 0>(p, RA, RX, nbr, cell0, tid);
     face_axis<D, M, VISC, AV, 1>(p, RA, RX, nbr, cell0, tid);
@@ -1041,7 +1070,10 @@ __global__ void __launch_bounds__((Cfg<D, M, VISC, AV>::NT), DG_STAGE_MINB) dg_s
     const int cell0 = blockIdx.x * C;
     // own modes of a full tile travel global -> RA as bulk asynchronous copies (one request per row segment);
     // with fewer than 8 cells per block (16/32-byte segments, m >= 6) batched plain loads are cheaper here
-    const bool bulk = (C >= 8) && bulk_ok<C>(cell0, p.ncells);
+    using GL = GLay<D, M>;
+    constexpr int RW = V * Np, RF = D * Vc * K::Nf;      // rows of a state array / of the flux array
+    const unsigned grs = GL::rs(p.ncells);
+    const bool bulk = (C >= 8) && GL::B == 0 && bulk_ok<C>(cell0, p.ncells);
     if (bulk) {
         if (tid == 0) mbar_init(bar, 1);
         __syncthreads();
@@ -1067,22 +1099,22 @@ __global__ void __launch_bounds__((Cfg<D, M, VISC, AV>::NT), DG_STAGE_MINB) dg_s
     double Fp[D][NLIFT], Fm[D][NLIFT];
 #pragma unroll
     for (int a = 0; a < D; ++a) {
-        const double *fp = p.flux + (size_t)(tid / C) * p.ncells + cg;
-        const double *fm = p.flux + (size_t)(tid / C) * p.ncells + nbm[a];
+        const double *fp = p.flux + (size_t)(tid / C) * grs + GL::cell(cg, RF);
+        const double *fm = p.flux + (size_t)(tid / C) * grs + GL::cell(nbm[a], RF);
 #pragma unroll
         for (int k = 0; k < NLIFT; ++k) {
             if (tid / C + k * (NT / C) < NFL) {
-                Fp[a][k] = __ldg(row_ptr(fp, a * NFL + k * (NT / C), p.ncells));
-                Fm[a][k] = __ldg(row_ptr(fm, a * NFL + k * (NT / C), p.ncells));
+                Fp[a][k] = __ldg(row_ptr(fp, a * NFL + k * (NT / C), grs));
+                Fm[a][k] = __ldg(row_ptr(fm, a * NFL + k * (NT / C), grs));
             }
         }
     }
     if (!p.rhs_only && cl % 4 == 0) {
         // u^n is needed only by the stage combine at the very end: start it towards L2 now
-        const double *wn = p.w_n + (size_t)(tid / C) * p.ncells + cg;
+        const double *wn = p.w_n + (size_t)(tid / C) * grs + GL::cell(cg, RW);
 #pragma unroll 4
         for (int k = 0; tid / C + k * (NT / C) < V * Np; ++k)
-            asm volatile("prefetch.global.L2 [%0];" ::"l"(row_ptr(wn, k * (NT / C), p.ncells)));
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(row_ptr(wn, k * (NT / C), grs)));
     }
     if (AV && tid < C) {
         // wiggle source of Eq. 45 from the previous step's sensor (readings A14, A15)
@@ -1095,7 +1127,7 @@ __global__ void __launch_bounds__((Cfg<D, M, VISC, AV>::NT), DG_STAGE_MINB) dg_s
     if (bulk)
         mbar_wait(bar, 0);
     else
-        load_own_modes<V, Np, C, NT, L>(p.w_prev, p.ncells, cg, RA, tid);   // global slot order: r = mode*V + v
+        load_own_modes<V, Np, C, NT, L>(p.w_prev + GL::cell(cg, RW), grs, RA, tid);   // global slot order: r = mode*V + v
     __syncthreads();
 
     // ---- surface term: lift the face fluxes of dg_face_kernel along each normal (Eq. 20, readings A3/A4) ----
@@ -1219,13 +1251,13 @@ __global__ void __launch_bounds__((Cfg<D, M, VISC, AV>::NT), DG_STAGE_MINB) dg_s
 #define LOAD_COMBINE_INPUTS()                                                                               \
     do {                                                                                                    \
         const bool need_n = !p.rhs_only, need_p = !p.rhs_only && p.rk_b != 0.0;                             \
-        const double *bn = p.w_n + (size_t)((tid / C) * V) * p.ncells + cg;                                 \
-        const double *bp = p.w_prev + (size_t)((tid / C) * V) * p.ncells + cg;                              \
+        const double *bn = p.w_n + (size_t)((tid / C) * V) * grs + GL::cell(cg, RW);                        \
+        const double *bp = p.w_prev + (size_t)((tid / C) * V) * grs + GL::cell(cg, RW);                     \
         _Pragma("unroll") for (int k = 0; k < CNK; ++k) _Pragma("unroll") for (int v = 0; v < V; ++v) {     \
             wn[k][v] = wp[k][v] = 0.0;                                                                      \
             if (tid / C + k * CG < Np) {                                                                    \
-                if (need_n) wn[k][v] = *row_ptr(bn, k * CG * V + v, p.ncells);    /* may alias w_out */                        \
-                if (need_p) wp[k][v] = __ldg(row_ptr(bp, k * CG * V + v, p.ncells));                        \
+                if (need_n) wn[k][v] = *row_ptr(bn, k * CG * V + v, grs);    /* may alias w_out */          \
+                if (need_p) wp[k][v] = __ldg(row_ptr(bp, k * CG * V + v, grs));                             \
             }                                                                                               \
         }                                                                                                   \
     } while (0)
@@ -1312,7 +1344,7 @@ __global__ void __launch_bounds__((Cfg<D, M, VISC, AV>::NT), DG_STAGE_MINB) dg_s
         constexpr int NK = CNK;
         const int g = tid / C;
         const bool active = cell0 + cl < p.ncells;
-        double *bo = p.w_out + (size_t)(g * V) * p.ncells + cg;
+        double *bo = p.w_out + (size_t)(g * V) * grs + GL::cell(cg, RW);
 #pragma unroll
         for (int k = 0; k < NK; ++k) {
             const int mode = g + k * G;
@@ -1333,10 +1365,10 @@ __global__ void __launch_bounds__((Cfg<D, M, VISC, AV>::NT), DG_STAGE_MINB) dg_s
                     const double Ld = keep ? ACC[L::at2(v, mode) * C + cl] : 0.0;
                     double wnew = Ld;
                     if (!p.rhs_only) wnew = fma(cdt, Ld, fma(p.rk_b, wp[k][v], p.rk_a * wn[k][v]));
-                    if (active) *row_ptr(bo, k * G * V + v, p.ncells) = wnew;
+                    if (active) *row_ptr(bo, k * G * V + v, grs) = wnew;
                     if (p.w_aux != nullptr && active) {
                         // SSPRK(5,4): the part of the last stage that is known now (u^(2), u^(3), L(u^(3)))
-                        const size_t gi = (size_t)((g + k * G) * V + v) * p.ncells + cg;
+                        const size_t gi = (size_t)((g + k * G) * V + v) * grs + GL::cell(cg, RW);
                         p.w_aux[gi] = fma(p.aux_c * p.scal[0], Ld, fma(p.aux_b, wp[k][v], p.aux_a * p.w_aux_in[gi]));
                     }
                     if (p.do_wavespeed) RA[L::at2(v, mode) * C + cl] = wnew;
@@ -1405,7 +1437,8 @@ __global__ void __launch_bounds__((Cfg<D, M, VISC, AV>::NT), DG_STAGE_MINB) dg_w
     double *red = RA + V * Np * C + K::RX * C + V * Np * C + C;
     const int tid = threadIdx.x;
     const int cell0 = blockIdx.x * C;
-    load_own_modes<V, Np, C, NT, L>(p.w_prev, p.ncells, min(cell0 + tid % C, p.ncells - 1), RA, tid);
+    load_own_modes<V, Np, C, NT, L>(p.w_prev + GLay<D, M>::cell(min(cell0 + tid % C, p.ncells - 1), V * Np),
+                                    GLay<D, M>::rs(p.ncells), RA, tid);
     __syncthreads();
     expand_volume<D, M, C, NT, K::BLK, L>(RA, Vc, tid);
     wavespeed_points<D, M, C, NT, L>(RA, p.gamma, p.flag, red, p.maxbits, tid);

@@ -73,8 +73,9 @@ cudaError_t launch(const DgStageArgs &a, cudaStream_t st, int wavespeed_only) {
 }
 
 template <bool VISC, bool AV>
-void info(int *c, int *nt, int *smem, int *fused_limiter) {
+void info(int *c, int *nt, int *smem, int *fused_limiter, int *bsz) {
     *fused_limiter = dgk::Cfg<DG_DIM, DG_M, VISC, AV>::PP ? 1 : 0;
+    *bsz = dgk::GLay<DG_DIM, DG_M>::B;
     using K = dgk::Cfg<DG_DIM, DG_M, VISC, AV>;
     if constexpr (K::PP) {
         using K2 = dgk::Cfg2<DG_DIM, DG_M, VISC, AV>;
@@ -110,11 +111,11 @@ cudaError_t DG_FN(dg_upload, DG_DIM, DG_M)(const DgTables *t) {
     return cudaMemcpyToSymbol(c_tab, t, sizeof(DgTables));
 }
 
-void DG_FN(dg_info, DG_DIM, DG_M)(int visc, int av, int *c, int *nt, int *smem, int *fused_limiter) {
-    if (visc && av) return info<true, true>(c, nt, smem, fused_limiter);
-    if (visc) return info<true, false>(c, nt, smem, fused_limiter);
-    if (av) return info<false, true>(c, nt, smem, fused_limiter);
-    return info<false, false>(c, nt, smem, fused_limiter);
+void DG_FN(dg_info, DG_DIM, DG_M)(int visc, int av, int *c, int *nt, int *smem, int *fused_limiter, int *bsz) {
+    if (visc && av) return info<true, true>(c, nt, smem, fused_limiter, bsz);
+    if (visc) return info<true, false>(c, nt, smem, fused_limiter, bsz);
+    if (av) return info<false, true>(c, nt, smem, fused_limiter, bsz);
+    return info<false, false>(c, nt, smem, fused_limiter, bsz);
 }
 
 cudaError_t DG_FN(dg_config, DG_DIM, DG_M)(int visc, int av) {

@@ -765,9 +765,9 @@ struct FaceCfg {
     // DIRECT (3D register-tile configurations): F1 reads the own modes straight from global memory / L1 like the
     // neighbour's (each is used once per axis), so no copy of the tile is staged in shared memory, the block does
     // not wait for it before the first axis, and only the face scratch remains (more cells or blocks per SM)
-    static constexpr bool DIRECT = DG_FACE_DIRECT && K::BLK && (D == 3);
+    static constexpr bool DIRECT = DG_FACE_DIRECT && ((K::BLK && D == 3) || GLay<D, M>::B > 0);
     static constexpr int FP = (DIRECT ? 0 : K::V * K::Np) + K::NQ * K::Nf;   // doubles per cell: [own modes +] one face
-    static constexpr int MINB = DIRECT ? DG_FACE_DIRECT_MINB : (BIG ? 1 : DG_FACE_MINB);   // resident blocks per SM (register cap)
+    static constexpr int MINB = BIG ? 1 : (DIRECT ? DG_FACE_DIRECT_MINB : DG_FACE_MINB);   // resident blocks per SM (register cap)
     static constexpr int CMAX = DIRECT ? 16 : 32;
     static constexpr int pick_c() {
         int c = CMAX;
@@ -802,32 +802,49 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA
         static_assert(NT % C == 0, "threads per block must be a multiple of cells per block");
         constexpr int NIT = (V * Nf * C + NT - 1) / NT;
         constexpr int NB = FK::DIRECT ? (NIT % 3 == 0 ? 3 : (NIT % 2 == 0 ? 2 : 1)) : NIT;   // items per load batch
-        const int cell = tid % C;
-        const int nc = nbr[A * C + cell];
-        const int oc = min(cell0 + cell, p.ncells - 1);
         using GL = GLay<D, M>;
+        // Block layout (GL::B > 0): items are numbered in memory order -- cell within its block fastest, then the
+        // variable, then the transverse mode -- so that the lanes of a warp read adjacent doubles (row = mode*V + v,
+        // address = row*B + cell % B); otherwise lanes = cells and the rows of a thread's items are NT/C apart.
+        constexpr bool MO = GL::B > 0;
+        constexpr int BB = MO ? GL::B : 1;
         const unsigned grs = GL::rs(p.ncells);
-        const double *wnb = p.w_prev + GL::cell(nc, V * K::Np), *wow = p.w_prev + GL::cell(oc, V * K::Np);
-        // the upper x neighbour of every cell but the last one of the tile is the next cell of the tile itself
-        const bool from_tile = !FK::DIRECT && (A == 0) && (cell < C - 1) && (cell0 + cell + 1 < p.ncells) &&
-                               (nc == cell0 + cell + 1);
+        auto item = [&](int k, int &cell, int &v, int &lt) -> bool {
+            if (MO) {
+                const int e = tid + k * NT;
+                cell = (e / (BB * V * Nf)) * BB + e % BB;
+                v = (e / BB) % V;
+                lt = (e / (BB * V)) % Nf;
+                return e < C * V * Nf;
+            }
+            const int r = tid / C + k * (NT / C);          // v*Nf + lt
+            cell = tid % C;
+            v = r / Nf;
+            lt = r % Nf;
+            return r < V * Nf;
+        };
 #pragma unroll
         for (int k0 = 0; k0 < NIT; k0 += NB) {
             double nb[NB][M], ow[NB][M];
 #pragma unroll
             for (int kk = 0; kk < NB; ++kk) {
-                const int r = tid / C + (k0 + kk) * (NT / C);          // v*Nf + lt
-                if (r < V * Nf) {
-                    const int base = pencil_base<M, SA>(r % Nf);
-                    const int v = r / Nf;
+                int cell, v, lt;
+                if (item(k0 + kk, cell, v, lt)) {
+                    const int base = pencil_base<M, SA>(lt);
+                    const int nc = nbr[A * C + cell];
+                    // the upper x neighbour of every cell but the last one of the tile is the next cell of the tile
+                    const bool from_tile = !FK::DIRECT && (A == 0) && (cell < C - 1) && (cell0 + cell + 1 < p.ncells) &&
+                                           (nc == cell0 + cell + 1);
                     if (from_tile) {
 #pragma unroll
                         for (int l = 0; l < M; ++l) nb[kk][l] = RA[LV::at2(v, base + l * SA) * C + cell + 1];
                     } else {
+                        const double *wnb = p.w_prev + GL::cell(nc, V * K::Np);
 #pragma unroll
                         for (int l = 0; l < M; ++l) nb[kk][l] = __ldg(row_ptr(wnb, (base + l * SA) * V + v, grs));
                     }
                     if (FK::DIRECT) {
+                        const double *wow = p.w_prev + GL::cell(min(cell0 + cell, p.ncells - 1), V * K::Np);
 #pragma unroll
                         for (int l = 0; l < M; ++l) ow[kk][l] = __ldg(row_ptr(wow, (base + l * SA) * V + v, grs));
                     }
@@ -835,10 +852,8 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA
             }
 #pragma unroll
             for (int kk = 0; kk < NB; ++kk) {
-                const int r = tid / C + (k0 + kk) * (NT / C);
-                if (r < V * Nf) {
-                    const int lt = r % Nf;
-                    const int v = r / Nf;
+                int cell, v, lt;
+                if (item(k0 + kk, cell, v, lt)) {
                     const int base = pencil_base<M, SA>(lt);
                     double own[M];
 #pragma unroll

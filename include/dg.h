@@ -15,7 +15,9 @@
  *  - Pointers named `w`, `alpha`, `totals`, `out` may be HOST or DEVICE pointers (detected with
  *    cudaPointerGetAttributes); they are caller-owned and only accessed during the call.  All device
  *    state is library-owned and released by dg_free().
- *  - State layout (external == internal for the conserved variables):
+ *  - State layout of every caller buffer (the library keeps the same layout internally, except in 3D with
+ *    order >= 6, where cells are stored in blocks of 2 or 4 so that the rows of a tile are adjacent in memory; the
+ *    conversion happens inside dg_set_state / dg_get_state / dg_eval_rhs / dg_set_alpha / dg_get_alpha):
  *        w[(mode*Vc + var)*Ncells + cell],  Vc = dim+2,
  *        cell = (iz*Ny + iy)*Nx + ix,  mode = (lz*m + ly)*m + lx,  m = order,
  *        var  = rho, rho v_x, rho v_y, (rho v_z), e      (Eq. 1-3).

@@ -21,13 +21,15 @@ Legendre values by three-term recurrence, every step in the paper's order and no
   O11 SSP-RK           PAPER.md:200 (Shu-Osher forms; 3-stage default per BASELINE config 1)
   O12 totals           PAPER.md:127, 423 (mode 0 is the cell mean)
   O13 positivity lim.  PAPER.md:417-432 (Eq. 47), optional, after every RK stage (readings L1-L6 in DESIGN.md)
+  O14 passive tracer   PAPER.md:325-329 (Eq. 40), optional extra row c rho: advective flux c rho v, HLLC row
+                       c_K x (star mass flux), diffusive flux eta rho grad c (readings T1-T3 in DESIGN.md)
 
 Parity pins (tests/test_oracle_*.py) cover every function here; the readings with no pin in the paper
 (A6, A11, A12, A14, A15, A18 in DESIGN.md) are "parity unpinned" against the authors' code but pinned as
 mathematics where a closed form exists (HLLC consistency/exact contact/Sod star state, etc.).
 
 State array layout inside the oracle: w[cell, mode, var]; cell = (iz*Ny+iy)*Nx+ix, mode = (lz*m+ly)*m+lx,
-var = rho, rho v_x, rho v_y, (rho v_z), e, [alpha].  The C-ABI layout w[(mode*Vc+var)*Ncells+cell]
+var = rho, rho v_x, rho v_y, (rho v_z), e, [c rho], [alpha].  The C-ABI layout w[(mode*Vc+var)*Ncells+cell]
  is converted in set_state/get_state.
 """
 from __future__ import annotations
@@ -147,6 +149,8 @@ def euler_flux(u, a: int, d: int, gamma: float):
         f[..., 1 + b] = rho * v[..., a] * v[..., b]
     f[..., 1 + a] += p
     f[..., 1 + d] = (u[..., 1 + d] + p) * v[..., a]
+    for k in range(d + 2, u.shape[-1]):          # passive tracer rows c rho (Eq. 40): flux c rho v_a
+        f[..., k] = u[..., k] * v[..., a]
     return f
 
 
@@ -176,6 +180,8 @@ def hllc_flux(uL, uR, a: int, d: int, gamma: float):
         for b in range(d):
             us[..., 1 + b] = fac * (Sstar if b == a else v[..., b])
         us[..., 1 + d] = fac * (u[..., 1 + d] / rho + (Sstar - vn) * (Sstar + p / (rho * (S - vn))))
+        for k in range(d + 2, u.shape[-1]):      # a passive scalar is carried like a transverse velocity (reading T1)
+            us[..., k] = fac * (u[..., k] / rho)
         return us
 
     UsL = star_state(uL, rhoL, vL, pL, vnL, SL)
@@ -188,7 +194,7 @@ def hllc_flux(uL, uR, a: int, d: int, gamma: float):
     return F
 
 
-def ns_flux(u, grad, a: int, d: int, gamma: float, nu: float, chi: float):
+def ns_flux(u, grad, a: int, d: int, gamma: float, nu: float, chi: float, eta: float = 0.0):
     """Navier-Stokes flux column a (Eq. 38-39), grad[b][..., var] = d u_var / d x_b:
       F_NS,a = (0, Pi_{a b}, sum_b v_b Pi_{a b} + chi (gamma-1) rho d_a u_th),
       Pi = nu rho (grad v + grad v^T - 2/3 (div v) I)   (traceless reading A7),
@@ -205,6 +211,10 @@ def ns_flux(u, grad, a: int, d: int, gamma: float, nu: float, chi: float):
     duth = grad[a][..., 1 + d] / rho - e * grad[a][..., 0] / (rho * rho) - sum(
         v[..., c] * dv[a][c] for c in range(d))
     F[..., 1 + d] += chi * (gamma - 1.0) * rho * duth
+    for k in range(d + 2, u.shape[-1]):
+        # tracer diffusion eta rho d_a c (Eq. 40), grad c = [grad(c rho) - c grad rho] / rho
+        c = u[..., k] / rho
+        F[..., k] = eta * rho * (grad[a][..., k] - c * grad[a][..., 0]) / rho
     return F
 
 
@@ -256,6 +266,9 @@ class Options:
     # mode set: "tensor" = all (n+1)^d products (reading A1, BASELINE.json mode counts); "total_degree" = the paper's
     # own set, products whose total degree sum_a l_a exceeds n are discarded (Eq. 17-18)
     basis: str = "tensor"
+    # passive tracer (Eq. 40): one more conserved row c rho behind the energy, diffusivity eta
+    tracer_enable: bool = False
+    eta: float = 0.0
 
 
 class DGOracle:
@@ -273,10 +286,12 @@ class DGOracle:
         self.nu = float(nu)
         self.chi = float(chi)
         self.opt = options if options is not None else Options()
-        self.Vc = d + 2
+        self.tracer = bool(self.opt.tracer_enable)
+        self.eta = float(self.opt.eta) if self.tracer else 0.0
+        self.Vc = d + 2 + (1 if self.tracer else 0)
         self.av = bool(self.opt.av_enable)
         self.V = self.Vc + (1 if self.av else 0)
-        self.visc = (self.nu > 0.0) or (self.chi > 0.0)
+        self.visc = (self.nu > 0.0) or (self.chi > 0.0) or (self.eta > 0.0)
         self.need_grad = self.visc or self.av
         self.M = m ** d
         self.Np = m ** d
@@ -434,7 +449,7 @@ class DGOracle:
         for a in range(d):
             G = euler_flux(u, a, d, gamma)
             if self.visc:
-                G = G - ns_flux(u, grad, a, d, gamma, self.nu, self.chi)
+                G = G - ns_flux(u, grad, a, d, gamma, self.nu, self.chi, self.eta)
             if self.av:
                 G = G - eps[..., None] * grad[a]                                   # Eq. 24
             vol[:, :, :Vc] += pref * np.einsum("j,cjv,jl->clv", self.gvol, G, self.dPhi[a])
@@ -474,7 +489,7 @@ class DGOracle:
                 if np.any(rt <= 0.0) or np.any(pt <= 0.0):
                     self.unphysical = True
                 if self.visc:
-                    Fh = Fh - ns_flux(utc, gt, a, d, gamma, self.nu, self.chi)
+                    Fh = Fh - ns_flux(utc, gt, a, d, gamma, self.nu, self.chi, self.eta)
                 if self.av:
                     cst = np.sqrt(gamma * pt / rt)
                     epst = np.clip(ut[..., Vc], 0.0, self.opt.alpha_max) * cst * h / (n + 1)   # A12

@@ -18,7 +18,7 @@
  *  - State layout of every caller buffer (the library keeps the same layout internally, except in 3D with
  *    order >= 6, where cells are stored in blocks of 2 or 4 so that the rows of a tile are adjacent in memory; the
  *    conversion happens inside dg_set_state / dg_get_state / dg_eval_rhs / dg_set_alpha / dg_get_alpha):
- *        w[(mode*Vc + var)*Ncells + cell],  Vc = dim+2,
+ *        w[(mode*Vc + var)*Ncells + cell],  Vc = dim+2 (dim+3 with the passive tracer: var dim+2 = c*rho, Eq. 40),
  *        cell = (iz*Ny + iy)*Nx + ix,  mode = (lz*m + ly)*m + lx,  m = order,
  *        var  = rho, rho v_x, rho v_y, (rho v_z), e      (Eq. 1-3).
  *    The artificial-viscosity field alpha is one more modal field, layout
@@ -70,6 +70,9 @@ typedef struct dg_options {
                           * total-degree set, products with l_x+l_y(+l_z) > n are discarded (Eq. 17-18):
                           * same storage layout, the discarded rows are zeroed by dg_set_state / dg_set_alpha and stay
                           * zero; the sensor of Eq. 42 then uses the modes with l_x+l_y(+l_z) = n */
+    int    tracer_enable; /* 1: carry a passive tracer (Eq. 40): one more conserved row c*rho behind
+                          * the energy, i.e. Vc = dim+3 in every state count and layout below; default 0 */
+    double eta;          /* tracer diffusivity of Eq. 40 (>= 0); default 0 */
 } dg_options;
 
 /* Fill *opt with the defaults above. */
@@ -136,6 +139,9 @@ int dg_get_alpha(dg_solver *s, double *alpha, size_t count);
  * totals[0] = mass, totals[1..dim] = momentum, totals[dim+1] = energy; unused entries are 0.
  * `totals` is a HOST pointer to 5 doubles.  Deterministic fixed-shape reduction. */
 int dg_conserved_totals(dg_solver *s, double totals[5]);
+/* |K| * sum_cells of the cell means of the tracer row c*rho (conserved by Eq. 40 on a periodic mesh); DG_EINVAL
+ * without tracer_enable.  `total` is a HOST pointer. */
+int dg_tracer_total(dg_solver *s, double *total);
 
 /* Evaluate dw/dt = L(w) (Eq. 20) of the current state without advancing it, for term-wise parity tests:
  * out has the layout of the state (count = Vc*M*Ncells); alpha_out (may be NULL) that of alpha. */

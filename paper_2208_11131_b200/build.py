@@ -2,7 +2,8 @@
 
     python -m paper_2208_11131_b200.build [--force]
 
-The stage kernel is compiled once per (dim, m) in parallel (16 translation units of dg_stage_inst.cu);
+The stage kernels are compiled once per (dim, m, tracer row or not) in parallel (32 translation units of
+dg_stage_inst.cu);
 objects land in paper_2208_11131_b200/build/ and are rebuilt only when a source is newer.
 """
 from __future__ import annotations
@@ -48,11 +49,12 @@ def build(force: bool = False, verbose: bool = False) -> str:
     nvcc = _nvcc()
     os.makedirs(OBJ, exist_ok=True)
     jobs = []
-    for d in (2, 3):
-        for m in range(1, 9):
-            o = os.path.join(OBJ, "stage_%d_%d.o" % (d, m))
-            jobs.append((o, [nvcc] + NVCC_FLAGS + ["-DDG_DIM=%d" % d, "-DDG_M=%d" % m, "-c",
-                                                  os.path.join(CSRC, "dg_stage_inst.cu"), "-o", o]))
+    for t in (0, 1):            # without / with the passive-tracer row
+        for d in (2, 3):
+            for m in range(1, 9):
+                o = os.path.join(OBJ, "stage_%d_%d%s.o" % (d, m, "_t1" if t else ""))
+                jobs.append((o, [nvcc] + NVCC_FLAGS + ["-DDG_DIM=%d" % d, "-DDG_M=%d" % m, "-DDG_TRACER=%d" % t, "-c",
+                                                      os.path.join(CSRC, "dg_stage_inst.cu"), "-o", o]))
     o = os.path.join(OBJ, "api.o")
     jobs.append((o, [nvcc] + NVCC_FLAGS + ["-c", os.path.join(CSRC, "dg_api.cu"), "-o", o]))
     o = os.path.join(OBJ, "tables.o")

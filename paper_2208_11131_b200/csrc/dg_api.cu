@@ -42,9 +42,13 @@ struct Dispatch {
     limit_fn limit;
 };
 
-#define DG_ENTRY(d, m) {DG_FN(dg_launch, d, m), DG_FN(dg_upload, d, m), DG_FN(dg_info, d, m), DG_FN(dg_config, d, m), \
-                        DG_FN(dg_limit, d, m)},
-const Dispatch kDispatch[2][8] = {{DG_FOR_ALL_M(DG_ENTRY, 2)}, {DG_FOR_ALL_M(DG_ENTRY, 3)}};
+#define DG_ENTRY_T(d, m, t) {DG_FNT(dg_launch, d, m, t), DG_FNT(dg_upload, d, m, t), DG_FNT(dg_info, d, m, t), \
+                             DG_FNT(dg_config, d, m, t), DG_FNT(dg_limit, d, m, t)},
+#define DG_ENTRY0(d, m) DG_ENTRY_T(d, m, 0)
+#define DG_ENTRY1(d, m) DG_ENTRY_T(d, m, 1)
+// [passive tracer off / on][dim - 2][order - 1]
+const Dispatch kDispatch[2][2][8] = {{{DG_FOR_ALL_M(DG_ENTRY0, 2)}, {DG_FOR_ALL_M(DG_ENTRY0, 3)}},
+                                     {{DG_FOR_ALL_M(DG_ENTRY1, 2)}, {DG_FOR_ALL_M(DG_ENTRY1, 3)}}};
 
 // ---- helper kernels -------------------------------------------------------------------------------
 
@@ -151,6 +155,8 @@ struct dg_solver {
     double h, gamma, nu, chi;
     dg_options opt;
     int visc, av, Vc, V, M;
+    int tracer;             // passive tracer row c rho behind the energy
+    double eta;             // its diffusivity
     size_t nstate;          // V * M * ncells doubles
     int B;                  // cells per block of the internal layout (0: structure of arrays = the C-ABI layout)
     int ncpad;              // ncells rounded up to a multiple of B
@@ -222,6 +228,8 @@ int validate(const dg_mesh *mesh, int order, double gamma, double nu, double chi
         return fail(DG_EINVAL, "rk_stages must be 1, 2, 3 or 5");
     if (!(o->f_cfl > 0.0) && !(o->fixed_dt > 0.0)) return fail(DG_EINVAL, "f_cfl must be positive");
     if (o->basis != 0 && o->basis != 1) return fail(DG_EINVAL, "basis must be 0 (tensor product) or 1 (total degree)");
+        if (o->tracer_enable != 0 && o->tracer_enable != 1) return fail(DG_EINVAL, "tracer_enable must be 0 or 1");
+        if (o->tracer_enable && !(o->eta >= 0.0)) return fail(DG_EINVAL, "eta (tracer diffusivity) must be non-negative");
     if (o->av_enable) {
         if (!(o->f_tau > 0.0)) return fail(DG_EINVAL, "f_tau must be positive (Eq. 44 divides by it)");
         if (!(o->f_v >= 0.0) || !(o->f_w >= 0.0)) return fail(DG_EINVAL, "f_v and f_w must be non-negative");
@@ -247,6 +255,7 @@ void fill_args(const dg_solver *s, DgStageArgs *a) {
     a->gamma = s->gamma;
     a->nu = s->nu;
     a->chi = s->chi;
+    a->eta = s->eta;
     a->f_v = s->opt.f_v;
     a->f_tau = s->opt.f_tau;
     a->f_w = s->opt.f_w;
@@ -399,14 +408,16 @@ int init_common(dg_solver **out, const dg_mesh *mesh, int order, double gamma, d
     s->nu = nu;
     s->chi = chi;
     s->opt = o;
-    s->visc = (nu > 0.0 || chi > 0.0) ? 1 : 0;
+    s->tracer = o.tracer_enable ? 1 : 0;
+    s->eta = s->tracer ? o.eta : 0.0;
+    s->visc = (nu > 0.0 || chi > 0.0 || s->eta > 0.0) ? 1 : 0;
     s->av = o.av_enable ? 1 : 0;
-    s->Vc = s->dim + 2;
+    s->Vc = s->dim + 2 + s->tracer;
     s->V = s->Vc + s->av;
     s->M = 1;
     for (int a = 0; a < s->dim; ++a) s->M *= order;
     s->nstate = (size_t)s->V * s->M * s->ncells;
-    s->fn = kDispatch[s->dim - 2][order - 1];
+    s->fn = kDispatch[s->tracer][s->dim - 2][order - 1];
     s->fn.info(s->visc, s->av, &s->kC, &s->kNT, &s->kSmem, &s->fused_limiter, &s->B);
     s->ncpad = s->B ? (s->ncells + s->B - 1) / s->B * s->B : s->ncells;
     s->nalloc = (size_t)s->V * s->M * s->ncpad;
@@ -516,6 +527,8 @@ int dg_default_options(dg_options *opt) {
     opt->use_graph = 1;
     opt->limiter_enable = 0;
     opt->basis = 0;
+    opt->tracer_enable = 0;
+    opt->eta = 0.0;
     return DG_OK;
 }
 
@@ -665,17 +678,35 @@ int dg_get_alpha(dg_solver *s, double *alpha, size_t count) {
     return DG_OK;
 }
 
-int dg_conserved_totals(dg_solver *s, double totals[5]) {
-    if (!s || !totals) return fail(DG_EINVAL, "NULL argument");
+namespace {
+int all_totals(dg_solver *s, double t[8]) {
     double vol = 1.0;
     for (int a = 0; a < s->dim; ++a) vol *= s->h;
     dg_totals_kernel<<<s->Vc, 1024, 0, s->stream>>>(s->W0, s->V, s->ncells, vol, s->scal + 8, s->B, (size_t)s->V * s->M);
     CU(cudaGetLastError());
     s->launches += 1;
-    double t[5] = {0, 0, 0, 0, 0};
     CU(cudaMemcpyAsync(t, s->scal + 8, s->Vc * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
     CU(cudaStreamSynchronize(s->stream));
-    for (int i = 0; i < 5; ++i) totals[i] = (i < s->Vc) ? t[i] : 0.0;
+    return DG_OK;
+}
+}  // namespace
+
+int dg_conserved_totals(dg_solver *s, double totals[5]) {
+    if (!s || !totals) return fail(DG_EINVAL, "NULL argument");
+    double t[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    int rc = all_totals(s, t);
+    if (rc) return rc;
+    for (int i = 0; i < 5; ++i) totals[i] = (i < s->dim + 2) ? t[i] : 0.0;
+    return DG_OK;
+}
+
+int dg_tracer_total(dg_solver *s, double *total) {
+    if (!s || !total) return fail(DG_EINVAL, "NULL argument");
+    if (!s->tracer) return fail(DG_EINVAL, "the passive tracer is not enabled");
+    double t[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    int rc = all_totals(s, t);
+    if (rc) return rc;
+    *total = t[s->dim + 2];
     return DG_OK;
 }
 
@@ -781,6 +812,8 @@ int dg_set_options(dg_solver *s, const dg_options *opt) {
     if (opt->rk_stages != s->opt.rk_stages || (opt->av_enable != 0) != (s->opt.av_enable != 0))
         return fail(DG_EINVAL, "rk_stages and av_enable fix the device buffers: create a new solver to change them");
     if (opt->basis != s->opt.basis) return fail(DG_EINVAL, "the mode set (basis) cannot change under a loaded state");
+    if ((opt->tracer_enable != 0) != (s->tracer != 0))
+        return fail(DG_EINVAL, "tracer_enable changes the state layout: create a new solver");
     dg_mesh m;
     std::memset(&m, 0, sizeof(m));
     m.dim = s->dim;
@@ -792,7 +825,10 @@ int dg_set_options(dg_solver *s, const dg_options *opt) {
     int rc = validate(&m, s->order, s->gamma, s->nu, s->chi, opt);
     if (rc) return rc;
     CU(cudaStreamSynchronize(s->stream));
+    if (s->tracer && ((opt->eta > 0.0) != (s->eta > 0.0)) && !(s->nu > 0.0 || s->chi > 0.0))
+        return fail(DG_EINVAL, "switching the tracer diffusivity on or off changes the kernel variant: create a new solver");
     s->opt = *opt;
+    if (s->tracer) s->eta = opt->eta;
     drop_graph(s);              // the captured step carries the old options
     s->speeds_valid = false;    // limiter on/off changes where the wave speeds are taken
     return DG_OK;

@@ -14,11 +14,11 @@
 
 #include "dg_stage.cuh"
 
-namespace dgk {
+namespace DG_NS {
 
 template <int D, int M>
 struct LimCfg {
-    static constexpr int Vc = D + 2;
+    static constexpr int Vc = D + 2 + DG_TRACER;
     static constexpr int Np = ipow(M, D);
     static constexpr int Nf = ipow(M, D - 1);
     static constexpr int NFS = 2 * D * Vc;                       // face slots: (axis, side, variable)
@@ -49,7 +49,7 @@ __device__ __forceinline__ double ord_dec(unsigned long long u) {
 // Scratch of the limiter per block of C cells (after the face point values).
 template <int D, int C>
 struct LimScratch {
-    static constexpr int Vc = D + 2;
+    static constexpr int Vc = D + 2 + DG_TRACER;
     double *mean, *Fc, *rbot, *pbot;
     unsigned long long *key;
     int *act;
@@ -72,7 +72,7 @@ struct LimScratch {
 template <int D, int M, int C, int NT, bool BLK, class LV>
 __device__ __forceinline__ void limiter_core(double *NV, double *NF, const LimScratch<D, C> &sc, double gamma, int *flag,
                                              int cell0, int ncells, int tid) {
-    constexpr int Vc = D + 2, Np = ipow(M, D), Nf = ipow(M, D - 1), NFS = 2 * D * Vc;
+    constexpr int Vc = D + 2 + DG_TRACER, Np = ipow(M, D), Nf = ipow(M, D - 1), NFS = 2 * D * Vc;
     constexpr int NPT = Np + 2 * D * Nf;                         // evaluation points per cell
     constexpr int G = NT / C;
     using LF = Lay<Nf, Nf, false, 0>;
@@ -215,4 +215,4 @@ __global__ void __launch_bounds__(256, 2) dg_limiter_kernel(double *w, int V, in
     }
 }
 
-}  // namespace dgk
+}  // namespace DG_NS

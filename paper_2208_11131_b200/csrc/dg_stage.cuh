@@ -29,6 +29,18 @@
 #define DG_SEL_S 2
 #define DG_SEL_VTG 3
 
+// passive tracer (Eq. 40): one more conserved row c rho behind the energy.  A compile-time switch of the
+// translation unit (dg_stage_inst.cu is built with -DDG_TRACER=0 and =1), so the default kernels are unchanged.
+#ifndef DG_TRACER
+#define DG_TRACER 0
+#endif
+// kernels of the two builds live in different namespaces: equal template instantiations from different translation
+// units would otherwise be merged by the linker
+#if DG_TRACER
+#define DG_NS dgkt
+#else
+#define DG_NS dgk
+#endif
 #ifndef DG_AOSOA
 #define DG_AOSOA 1
 #endif
@@ -66,7 +78,7 @@
 
 __constant__ DgTables c_tab;
 
-namespace dgk {
+namespace DG_NS {
 
 __host__ __device__ constexpr int ipow(int b, int e) { return e <= 0 ? 1 : b * ipow(b, e - 1); }
 __host__ __device__ constexpr int imax(int a, int b) { return a > b ? a : b; }
@@ -77,7 +89,7 @@ constexpr int kSmemMax = 227 * 1024;
 template <int D, int M, bool VISC, bool AV>
 struct Cfg {
     static constexpr bool GRAD = VISC || AV;
-    static constexpr int Vc = D + 2;
+    static constexpr int Vc = D + 2 + DG_TRACER;
     static constexpr int V = Vc + (AV ? 1 : 0);
     static constexpr int Np = ipow(M, D);
     static constexpr int Nf = ipow(M, D - 1);
@@ -448,6 +460,7 @@ __device__ __forceinline__ void euler_flux(const double *u, const Prim<D> &q, in
 #pragma unroll
     for (int b = 0; b < D; ++b) f[1 + b] = u[1 + a] * q.v[b] + (b == a ? q.p : 0.0);
     f[1 + D] = (q.e + q.p) * va;
+    if (DG_TRACER) f[2 + D] = u[2 + D] * va;      // c rho v_a (Eq. 40)
 }
 
 // HLLC flux along axis a (Toro's HLLC with Davis wave-speed bounds, reading A6)
@@ -477,7 +490,7 @@ __device__ __forceinline__ void hllc_flux(const double *uL, const double *uR, co
     const double S = left ? SL : SR;
     const double vn = left ? vnL : vnR;
     const double mK = left ? mL : mR;
-    double f[D + 2];
+    double f[D + 2 + DG_TRACER];
     euler_flux<D>(u, K, a, f);
     const double fac = mK * fast_rcp(S - Sstar);
     F[0] = f[0] + S * (fac - u[0]);
@@ -488,11 +501,13 @@ __device__ __forceinline__ void hllc_flux(const double *uL, const double *uR, co
     }
     const double es = fac * (K.e * K.ir + (Sstar - vn) * (Sstar + K.p * fast_rcp(mK)));
     F[1 + D] = f[1 + D] + S * (es - K.e);
+    // a passive scalar is carried like a transverse velocity (reading T1): U*_K row = fac c_K
+    if (DG_TRACER) F[2 + D] = f[2 + D] + S * (fac * (u[2 + D] * K.ir) - u[2 + D]);
 }
 
 // velocity gradient dv[b][c] = d v_c / d x_b = (d_b(rho v_c) - v_c d_b rho) / rho
 template <int D>
-__device__ __forceinline__ void velocity_gradient(const Prim<D> &q, const double (*g)[D + 2], double (*dv)[D]) {
+__device__ __forceinline__ void velocity_gradient(const Prim<D> &q, const double (*g)[D + 2 + DG_TRACER], double (*dv)[D]) {
 #pragma unroll
     for (int b = 0; b < D; ++b)
 #pragma unroll
@@ -501,8 +516,9 @@ __device__ __forceinline__ void velocity_gradient(const Prim<D> &q, const double
 
 // Navier-Stokes flux column a (Eq. 38-39, traceless Pi, reading A7), SUBTRACTED from F
 template <int D>
-__device__ __forceinline__ void ns_flux_sub(const Prim<D> &q, const double (*g)[D + 2], const double (*dv)[D],
-                                            double divv, int a, double gamma, double nu, double chi, double *F) {
+__device__ __forceinline__ void ns_flux_sub(const Prim<D> &q, const double (*g)[D + 2 + DG_TRACER], const double (*dv)[D],
+                                            double divv, int a, double gamma, double nu, double chi, double *F,
+                                            double ctr = 0.0, double eta = 0.0) {
     double evisc = 0.0;
 #pragma unroll
     for (int b = 0; b < D; ++b) {
@@ -515,6 +531,8 @@ __device__ __forceinline__ void ns_flux_sub(const Prim<D> &q, const double (*g)[
     for (int c = 0; c < D; ++c) vdv = fma(q.v[c], dv[a][c], vdv);
     const double duth = g[a][1 + D] * q.ir - q.e * g[a][0] * (q.ir * q.ir) - vdv;
     F[1 + D] -= evisc + chi * (gamma - 1.0) * q.rho * duth;
+    // tracer diffusion eta rho d_a c, grad c = [grad(c rho) - c grad rho] / rho (Eq. 40); ctr = c at this point
+    if (DG_TRACER) F[2 + D] -= eta * (g[a][2 + D] - ctr * g[a][0]);
 }
 
 __device__ __forceinline__ void atomic_max_nonneg(unsigned long long *addr, double val) {
@@ -941,7 +959,7 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA
             bad |= !(qL.rho > 0.0) || !(qL.p > 0.0) || !(qR.rho > 0.0) || !(qR.p > 0.0);
             hllc_flux<D>(uL, uR, qL, qR, A, p.gamma, Fh);
             if (GRAD) {
-                double ut[Vc], g[D][D + 2];
+                double ut[Vc], g[D][D + 2 + DG_TRACER];
 #pragma unroll
                 for (int v = 0; v < Vc; ++v) {
                     ut[v] = RX[LF::at2(oUT + v, k) * C + cell];
@@ -959,7 +977,7 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA
                     double divv = 0.0;
 #pragma unroll
                     for (int b = 0; b < D; ++b) divv += dv[b][b];
-                    ns_flux_sub<D>(qt, g, dv, divv, A, p.gamma, p.nu, p.chi, Fh);
+                    ns_flux_sub<D>(qt, g, dv, divv, A, p.gamma, p.nu, p.chi, Fh, DG_TRACER ? ut[Vc - 1] * qt.ir : 0.0, p.eta);
                 }
                 if (AV) {
                     const double al = RX[LF::at2(oUT + Vc, k) * C + cell];
@@ -1211,7 +1229,7 @@ __global__ void __launch_bounds__((Cfg<D, M, VISC, AV>::NT), DG_STAGE_MINB) dg_s
             for (int v = 0; v < Vc; ++v) u[v] = RA[L::at2(v, j) * C + cell];
             const Prim<D> q = primitives<D>(u, p.gamma);
             bad |= !(q.rho > 0.0) || !(q.p > 0.0);
-            double g[D][D + 2], dv[D][D];
+            double g[D][D + 2 + DG_TRACER], dv[D][D];
             double divv = 0.0, eps = 0.0;
             if (GRAD) {
 #pragma unroll
@@ -1235,7 +1253,7 @@ __global__ void __launch_bounds__((Cfg<D, M, VISC, AV>::NT), DG_STAGE_MINB) dg_s
             for (int a = 0; a < D; ++a) {
                 double F[Vc];
                 euler_flux<D>(u, q, a, F);
-                if (VISC) ns_flux_sub<D>(q, g, dv, divv, a, p.gamma, p.nu, p.chi, F);
+                if (VISC) ns_flux_sub<D>(q, g, dv, divv, a, p.gamma, p.nu, p.chi, F, DG_TRACER ? u[Vc - 1] * q.ir : 0.0, p.eta);
                 if (AV) {
 #pragma unroll
                     for (int v = 0; v < Vc; ++v) F[v] -= eps * g[a][v];
@@ -1459,4 +1477,4 @@ __global__ void __launch_bounds__((Cfg<D, M, VISC, AV>::NT), DG_STAGE_MINB) dg_w
     wavespeed_points<D, M, C, NT, L>(RA, p.gamma, p.flag, red, p.maxbits, tid);
 }
 
-}  // namespace dgk
+}  // namespace DG_NS

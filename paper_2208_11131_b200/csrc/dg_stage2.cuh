@@ -35,7 +35,7 @@
 #define DG_S2_UNROLL_B 3
 #endif
 
-namespace dgk {
+namespace DG_NS {
 
 template <int D, int M, bool VISC, bool AV>
 struct Cfg2 {
@@ -49,7 +49,7 @@ struct Cfg2 {
     static constexpr int FP = V * Np + D * Vc * Np;
     // Wk[c], wave-speed scratch, sensor partials, S table
     // ... and the positivity limiter's per-cell scratch (fused form, see the kernel's tail)
-    static constexpr int lim_doubles(int c) { return (D + 2 + 3) * c + c + (c + 1) / 2 + 2 + (D + 2) * c; }
+    static constexpr int lim_doubles(int c) { return (K::Vc + 3) * c + c + (c + 1) / 2 + 2 + K::Vc * c; }
     static constexpr int extra_doubles(int c) {
         return c + 2 * (NT / 32) + (AV ? 4 * (NT / 32) * c : 0) + M * M + 2 + lim_doubles(c);
     }
@@ -194,7 +194,7 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
                 bad |= !(q.rho > 0.0) || !(q.p > 0.0);
                 // the gradient arrays hold d/dxi (reference coordinates): the factor 2/h of the cell map is folded
                 // into the two scalars that multiply them, 1/rho (velocity and temperature gradients) and eps
-                double g[D][D + 2], dv[D][D];
+                double g[D][D + 2 + DG_TRACER], dv[D][D];
                 double divv = 0.0, epss = 0.0;
                 const double gs = 2.0 * ih;
                 const double irs = q.ir * gs;
@@ -254,6 +254,8 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
                             ev = fma(q.v[b], Pi[a][b], ev);
                         }
                         F[1 + D] -= ev;
+                        // tracer diffusion eta rho d_a c (Eq. 40); the gradient arrays are in reference coordinates
+                        if (DG_TRACER) F[Vc - 1] -= p.eta * gs * (g[a][Vc - 1] - (u[Vc - 1] * q.ir) * g[a][0]);
                     }
                     if (AV) {
 #pragma unroll
@@ -578,4 +580,4 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
     }
 }
 
-}  // namespace dgk
+}  // namespace DG_NS

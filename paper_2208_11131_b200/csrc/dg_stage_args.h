@@ -16,6 +16,7 @@ struct DgStageArgs {
     double *sens_new;       // same, written on stage 1, committed to sens_prev on the last stage
     int ncells, nx, ny, nz;
     double h, gamma, nu, chi;
+    double eta;               // tracer diffusivity (DG_TRACER builds only)
     double f_v, f_tau, f_w, s_onset, alpha_max;
     double rk_a, rk_b, rk_c;  // u^(i) = rk_a u^n + rk_b u^(i-1) + rk_c dt L(u^(i-1))
     double aux_a, aux_b, aux_c;

@@ -14,59 +14,59 @@ namespace {
 // opt in to > 48 KB of dynamic shared memory (once per device context, outside any stream capture)
 template <bool VISC, bool AV>
 cudaError_t configure() {
-    using K = dgk::Cfg<DG_DIM, DG_M, VISC, AV>;
-    cudaError_t e = cudaFuncSetAttribute(dgk::dg_stage_kernel<DG_DIM, DG_M, VISC, AV>,
+    using K = DG_NS::Cfg<DG_DIM, DG_M, VISC, AV>;
+    cudaError_t e = cudaFuncSetAttribute(DG_NS::dg_stage_kernel<DG_DIM, DG_M, VISC, AV>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, K::kSmemBytes);
     if (e != cudaSuccess) return e;
     // NB: a kernel template must only ever be instantiated in the translation unit of its own (dim, m): every unit
     // has its own __constant__ tables, and the host stubs of equal instantiations are merged by the linker
     if constexpr (K::PP) {
-        e = cudaFuncSetAttribute(dgk::dg_stage2_kernel<DG_DIM, DG_M, VISC, AV, false>,
+        e = cudaFuncSetAttribute(DG_NS::dg_stage2_kernel<DG_DIM, DG_M, VISC, AV, false>,
                                  cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 dgk::Cfg2<DG_DIM, DG_M, VISC, AV>::kSmemBytes);
+                                 DG_NS::Cfg2<DG_DIM, DG_M, VISC, AV>::kSmemBytes);
         if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(dgk::dg_stage2_kernel<DG_DIM, DG_M, VISC, AV, true>,
+        e = cudaFuncSetAttribute(DG_NS::dg_stage2_kernel<DG_DIM, DG_M, VISC, AV, true>,
                                  cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 dgk::Cfg2<DG_DIM, DG_M, VISC, AV>::kSmemBytes);
+                                 DG_NS::Cfg2<DG_DIM, DG_M, VISC, AV>::kSmemBytes);
         if (e != cudaSuccess) return e;
     }
-    e = cudaFuncSetAttribute(dgk::dg_face_kernel<DG_DIM, DG_M, VISC, AV>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             dgk::FaceCfg<DG_DIM, DG_M, VISC, AV>::kSmemBytes);
+    e = cudaFuncSetAttribute(DG_NS::dg_face_kernel<DG_DIM, DG_M, VISC, AV>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             DG_NS::FaceCfg<DG_DIM, DG_M, VISC, AV>::kSmemBytes);
     if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(dgk::dg_limiter_kernel<DG_DIM, DG_M>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             dgk::LimCfg<DG_DIM, DG_M>::kSmemBytes);
+    e = cudaFuncSetAttribute(DG_NS::dg_limiter_kernel<DG_DIM, DG_M>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             DG_NS::LimCfg<DG_DIM, DG_M>::kSmemBytes);
     if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(dgk::dg_wavespeed_kernel<DG_DIM, DG_M, VISC, AV>,
+    return cudaFuncSetAttribute(DG_NS::dg_wavespeed_kernel<DG_DIM, DG_M, VISC, AV>,
                                 cudaFuncAttributeMaxDynamicSharedMemorySize, K::kSmemBytes);
 }
 
 template <bool VISC, bool AV>
 cudaError_t launch(const DgStageArgs &a, cudaStream_t st, int wavespeed_only) {
-    using K = dgk::Cfg<DG_DIM, DG_M, VISC, AV>;
+    using K = DG_NS::Cfg<DG_DIM, DG_M, VISC, AV>;
     const int blocks = (a.ncells + K::C - 1) / K::C;
     // wavespeed_only: 0 = face + stage kernels, 1 = wave-speed kernel, 2 = face kernel only, 3 = stage kernel only
     if (wavespeed_only == 1) {
-        dgk::dg_wavespeed_kernel<DG_DIM, DG_M, VISC, AV><<<blocks, K::NT, K::kSmemBytes, st>>>(a);
+        DG_NS::dg_wavespeed_kernel<DG_DIM, DG_M, VISC, AV><<<blocks, K::NT, K::kSmemBytes, st>>>(a);
         return cudaGetLastError();
     }
     if (wavespeed_only != 3) {
-        using FK = dgk::FaceCfg<DG_DIM, DG_M, VISC, AV>;
-        const dim3 fgrid = dgk::tile_grid<DG_DIM, FK::C>(a.ncells, a.nx, a.ny, a.nz);
-        dgk::dg_face_kernel<DG_DIM, DG_M, VISC, AV><<<fgrid, FK::NT, FK::kSmemBytes, st>>>(a);
+        using FK = DG_NS::FaceCfg<DG_DIM, DG_M, VISC, AV>;
+        const dim3 fgrid = DG_NS::tile_grid<DG_DIM, FK::C>(a.ncells, a.nx, a.ny, a.nz);
+        DG_NS::dg_face_kernel<DG_DIM, DG_M, VISC, AV><<<fgrid, FK::NT, FK::kSmemBytes, st>>>(a);
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
     if (wavespeed_only != 2) {
         if constexpr (K::PP) {
             // register-tile configurations (2 <= m <= 5): second-generation stage kernel (dg_stage2.cuh)
-            using K2 = dgk::Cfg2<DG_DIM, DG_M, VISC, AV>;
-            const dim3 grid2 = dgk::tile_grid<DG_DIM, K2::C>(a.ncells, a.nx, a.ny, a.nz);
+            using K2 = DG_NS::Cfg2<DG_DIM, DG_M, VISC, AV>;
+            const dim3 grid2 = DG_NS::tile_grid<DG_DIM, K2::C>(a.ncells, a.nx, a.ny, a.nz);
             if (!a.rhs_only && !a.total_degree && a.w_aux == nullptr)
-                dgk::dg_stage2_kernel<DG_DIM, DG_M, VISC, AV, true><<<grid2, K2::NT, K2::kSmemBytes, st>>>(a);
+                DG_NS::dg_stage2_kernel<DG_DIM, DG_M, VISC, AV, true><<<grid2, K2::NT, K2::kSmemBytes, st>>>(a);
             else
-                dgk::dg_stage2_kernel<DG_DIM, DG_M, VISC, AV, false><<<grid2, K2::NT, K2::kSmemBytes, st>>>(a);
+                DG_NS::dg_stage2_kernel<DG_DIM, DG_M, VISC, AV, false><<<grid2, K2::NT, K2::kSmemBytes, st>>>(a);
         } else {
-            dgk::dg_stage_kernel<DG_DIM, DG_M, VISC, AV><<<blocks, K::NT, K::kSmemBytes, st>>>(a);
+            DG_NS::dg_stage_kernel<DG_DIM, DG_M, VISC, AV><<<blocks, K::NT, K::kSmemBytes, st>>>(a);
         }
     }
     return cudaGetLastError();
@@ -74,11 +74,11 @@ cudaError_t launch(const DgStageArgs &a, cudaStream_t st, int wavespeed_only) {
 
 template <bool VISC, bool AV>
 void info(int *c, int *nt, int *smem, int *fused_limiter, int *bsz) {
-    *fused_limiter = dgk::Cfg<DG_DIM, DG_M, VISC, AV>::PP ? 1 : 0;
-    *bsz = dgk::GLay<DG_DIM, DG_M>::B;
-    using K = dgk::Cfg<DG_DIM, DG_M, VISC, AV>;
+    *fused_limiter = DG_NS::Cfg<DG_DIM, DG_M, VISC, AV>::PP ? 1 : 0;
+    *bsz = DG_NS::GLay<DG_DIM, DG_M>::B;
+    using K = DG_NS::Cfg<DG_DIM, DG_M, VISC, AV>;
     if constexpr (K::PP) {
-        using K2 = dgk::Cfg2<DG_DIM, DG_M, VISC, AV>;
+        using K2 = DG_NS::Cfg2<DG_DIM, DG_M, VISC, AV>;
         *c = K2::C;
         *nt = K2::NT;
         *smem = K2::kSmemBytes;
@@ -101,9 +101,9 @@ cudaError_t DG_FN(dg_launch, DG_DIM, DG_M)(int visc, int av, const DgStageArgs *
 
 // positivity limiter on a state buffer with V variables per mode (only the d+2 conserved ones are touched)
 cudaError_t DG_FN(dg_limit, DG_DIM, DG_M)(double *w, int V, int ncells, double gamma, int *flag, cudaStream_t st) {
-    using LK = dgk::LimCfg<DG_DIM, DG_M>;
+    using LK = DG_NS::LimCfg<DG_DIM, DG_M>;
     const int blocks = (ncells + LK::C - 1) / LK::C;
-    dgk::dg_limiter_kernel<DG_DIM, DG_M><<<blocks, LK::NT, LK::kSmemBytes, st>>>(w, V, ncells, gamma, flag);
+    DG_NS::dg_limiter_kernel<DG_DIM, DG_M><<<blocks, LK::NT, LK::kSmemBytes, st>>>(w, V, ncells, gamma, flag);
     return cudaGetLastError();
 }
 

@@ -33,7 +33,8 @@ class dg_mesh(C.Structure):
 class dg_options(C.Structure):
     _fields_ = [("f_cfl", C.c_double), ("rk_stages", C.c_int), ("av_enable", C.c_int), ("f_v", C.c_double),
                 ("f_tau", C.c_double), ("f_w", C.c_double), ("s_onset0", C.c_double), ("alpha_max", C.c_double),
-                ("fixed_dt", C.c_double), ("use_graph", C.c_int), ("limiter_enable", C.c_int), ("basis", C.c_int)]
+                ("fixed_dt", C.c_double), ("use_graph", C.c_int), ("limiter_enable", C.c_int), ("basis", C.c_int),
+                ("tracer_enable", C.c_int), ("eta", C.c_double)]
 
 
 class dg_diagnostics(C.Structure):
@@ -59,6 +60,7 @@ SYMBOLS = {
     "dg_get_state": (C.c_int, [_P, _P, C.c_size_t]),
     "dg_get_alpha": (C.c_int, [_P, _P, C.c_size_t]),
     "dg_conserved_totals": (C.c_int, [_P, C.POINTER(C.c_double * 5)]),
+    "dg_tracer_total": (C.c_int, [_P, C.POINTER(C.c_double)]),
     "dg_eval_rhs": (C.c_int, [_P, _P, C.c_size_t, _P, C.c_size_t]),
     "dg_get_time": (C.c_int, [_P, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
     "dg_set_options": (C.c_int, [_P, C.POINTER(dg_options)]),
@@ -135,9 +137,9 @@ class Solver:
         self.dim, self.order, self.h = int(dim), int(order), float(h)
         self.ncell = tuple(int(c) for c in ncell[:dim])
         self.ncells = int(np.prod(self.ncell))
-        self.Vc = dim + 2
         self.M = order ** dim
         self.opt = options if options is not None else default_options()
+        self.Vc = dim + 2 + (1 if self.opt.tracer_enable else 0)
         mesh = dg_mesh()
         mesh.dim = dim
         for a in range(3):
@@ -198,7 +200,12 @@ class Solver:
     def conserved_totals(self):
         t = (C.c_double * 5)()
         _check(self._lib.dg_conserved_totals(self._h, C.byref(t)))
-        return np.array(t[:self.Vc])
+        return np.array(t[:self.dim + 2])
+
+    def tracer_total(self):
+        t = C.c_double()
+        _check(self._lib.dg_tracer_total(self._h, C.byref(t)))
+        return t.value
 
     def eval_rhs(self, with_alpha=False, out=None, alpha_out=None):
         """dw/dt of the current state.  `out` / `alpha_out` may be numpy arrays or torch tensors (host or cuda)."""

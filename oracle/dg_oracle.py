@@ -25,7 +25,7 @@ Legendre values by three-term recurrence, every step in the paper's order and no
                        c_K x (star mass flux), diffusive flux eta rho grad c (readings T1-T3 in DESIGN.md)
 
 Parity pins (tests/test_oracle_*.py) cover every function here; the readings with no pin in the paper
-(A6, A11, A12, A14, A15, A18 in DESIGN.md) are "parity unpinned" against the authors' code but pinned as
+(A6, A11, A12, A14, A15, A18, L2, L3, A19b, T1, T2 in DESIGN.md) are "parity unpinned" against the authors' code but pinned as
 mathematics where a closed form exists (HLLC consistency/exact contact/Sod star state, etc.).
 
 State array layout inside the oracle: w[cell, mode, var]; cell = (iz*Ny+iy)*Nx+ix, mode = (lz*m+ly)*m+lx,

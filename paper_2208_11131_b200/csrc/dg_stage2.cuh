@@ -12,8 +12,8 @@
 //   * blocks walk the mesh in (y,z)-blocked order (tile_of_block) so that the lower y and z neighbours' face fluxes
 //     are still in L2 when they are read.
 // The face kernel writes the face fluxes in the matching partially projected form (Cfg::PP in dg_stage.cuh).
-// Measured dead ends (profiles/r2_stage_experiments.md): persistent blocks with the next tile's modes staged by TMA
-// tensor copies, L2 prefetch hints, 12 warps per block -- all slower than this form.
+// Measured dead ends (profiles/r2b_cfg4.md and earlier sessions of this round): persistent blocks with the next tile's
+// modes staged by TMA tensor copies, L2 prefetch hints, 12 warps per block, two 8-cell blocks per SM -- all slower.
 #pragma once
 
 #include "dg_stage.cuh"

@@ -160,6 +160,40 @@ struct Lay {
         if (SWZ) return slot * NPTS + (j ^ ((j / PL + slot) & 1));
         return slot * NPTS + rot(j);
     }
+    // point indices (inside a slot) of the M points of pencil `pen` along an axis of stride STRIDE.  With the row
+    // rotation the row index modulo M is known per axis (x sweep: the pencil's row; y sweep: the point's own y = i;
+    // z sweep: the pencil's y), so one division per pencil replaces two per point (m = 6: divisions by 6 were 80 %
+    // of the stage kernel's instructions).  Not for SWZ layouts (their exchange depends on the slot).
+    template <int M, int STRIDE>
+    static __device__ __forceinline__ void pencil(int pen, int *idx) {
+        if (ROTM > 0 && !SWZ) {
+            const int lo = pen % M, hi = pen / M;
+            if (STRIDE == 1) {                      // pen = row, lo = row % M
+#pragma unroll
+                for (int i = 0; i < M; ++i) {
+                    int x = i + lo;
+                    if (x >= M) x -= M;
+                    idx[i] = pen * M + x;
+                }
+            } else if (STRIDE == M) {               // pen = plane * M + x; point i sits in row plane * M + i
+#pragma unroll
+                for (int i = 0; i < M; ++i) {
+                    int x = lo + i;
+                    if (x >= M) x -= M;
+                    idx[i] = hi * M * M + i * M + x;
+                }
+            } else {                                // pen = y * M + x; every point sits in a row with row % M = y
+                int x = lo + hi;
+                if (x >= M) x -= M;
+#pragma unroll
+                for (int i = 0; i < M; ++i) idx[i] = i * STRIDE + hi * M + x;
+            }
+        } else {
+            const int pb = (pen / STRIDE) * (STRIDE * M) + (pen % STRIDE);
+#pragma unroll
+            for (int i = 0; i < M; ++i) idx[i] = rot(pb + i * STRIDE);
+        }
+    }
     // parity of tile g (PL points per tile): rows q and q^1 of the tile are exchanged when it is 1
     static __device__ __forceinline__ int tile_par(int g) {
         return SWZ ? ((g + (NPTS > PL ? g / (NPTS / PL) : 0)) & 1) : 0;
@@ -329,16 +363,21 @@ __device__ __forceinline__ void sweep(const double *src, int s0, int sum_slots, 
     }
     const int cell = tid % C;
     const int total = nslots * NPEN;
+    constexpr bool FASTIDX = !use_swizzle(M, C);      // SWZ layouts exchange rows depending on the slot: generic path
     for (int r = tid / C; r < total; r += NT / C) {
         const int pen = r % NPEN;
         const int slot = r / NPEN;
         const int pb = pencil_base<M, STRIDE>(pen);
+        int idx[M];
+        if (FASTIDX) L::template pencil<M, STRIDE>(pen, idx);
         double in[M];
 #pragma unroll
         for (int i = 0; i < M; ++i) {
-            in[i] = src[L::at2(s0 + slot, pb + i * STRIDE) * C + cell];
+            in[i] = FASTIDX ? src[((s0 + slot) * NPTS + idx[i]) * C + cell] : src[L::at2(s0 + slot, pb + i * STRIDE) * C + cell];
 #pragma unroll
-            for (int k = 1; k < NSUM; ++k) in[i] += src[L::at2(s0 + k * sum_slots + slot, pb + i * STRIDE) * C + cell];
+            for (int k = 1; k < NSUM; ++k)
+                in[i] += FASTIDX ? src[((s0 + k * sum_slots + slot) * NPTS + idx[i]) * C + cell]
+                                 : src[L::at2(s0 + k * sum_slots + slot, pb + i * STRIDE) * C + cell];
         }
         double res[M];
         apply1d<SEL, M>(in, res);
@@ -346,7 +385,7 @@ __device__ __forceinline__ void sweep(const double *src, int s0, int sum_slots, 
         for (int j = 0; j < M; ++j) {
             double acc = res[j];
             if (SCALE) acc *= scale;
-            double *d = dst + L::at2(d0 + slot, pb + j * STRIDE) * C + cell;
+            double *d = FASTIDX ? dst + ((d0 + slot) * NPTS + idx[j]) * C + cell : dst + L::at2(d0 + slot, pb + j * STRIDE) * C + cell;
             if (ADD)
                 *d += acc;
             else

@@ -896,14 +896,16 @@ __device__ __forceinline__ void face_axis(const DgStageArgs &p, const double *RA
 #pragma unroll
                         for (int l = 0; l < M; ++l) nb[kk][l] = RA[LV::at2(v, base + l * SA) * C + cell + 1];
                     } else {
-                        const double *wnb = p.w_prev + GL::cell(nc, V * K::Np);
+                        // one IMAD.WIDE per load: base pointer of (first row of the pencil, cell), compile-time row steps
+                        const double *wnb = row_ptr(p.w_prev + GL::cell(nc, V * K::Np), base * V + v, grs);
 #pragma unroll
-                        for (int l = 0; l < M; ++l) nb[kk][l] = __ldg(row_ptr(wnb, (base + l * SA) * V + v, grs));
+                        for (int l = 0; l < M; ++l) nb[kk][l] = __ldg(row_ptr(wnb, l * SA * V, grs));
                     }
                     if (FK::DIRECT) {
-                        const double *wow = p.w_prev + GL::cell(min(cell0 + cell, p.ncells - 1), V * K::Np);
+                        const double *wow =
+                            row_ptr(p.w_prev + GL::cell(min(cell0 + cell, p.ncells - 1), V * K::Np), base * V + v, grs);
 #pragma unroll
-                        for (int l = 0; l < M; ++l) ow[kk][l] = __ldg(row_ptr(wow, (base + l * SA) * V + v, grs));
+                        for (int l = 0; l < M; ++l) ow[kk][l] = __ldg(row_ptr(wow, l * SA * V, grs));
                     }
                 }
             }

@@ -286,12 +286,13 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
             if (g < Vc * NTILE) {
                 const double *fx = p.flux + (size_t)((0 * Vc + v) * Nf + jz * M) * p.ncells;
                 const double *fy = p.flux + (size_t)((1 * Vc + v) * Nf + jz * M) * p.ncells;
+                const double *fx0 = fx + cg, *fx1 = fx + nbm[0], *fy0 = fy + cg, *fy1 = fy + nbm[1];
 #pragma unroll
                 for (int i = 0; i < M; ++i) {
-                    gf[k][0][i] = __ldg(row_ptr(fx, i, p.ncells) + cg);
-                    gf[k][1][i] = __ldg(row_ptr(fx, i, p.ncells) + nbm[0]);
-                    gf[k][2][i] = __ldg(row_ptr(fy, i, p.ncells) + cg);
-                    gf[k][3][i] = __ldg(row_ptr(fy, i, p.ncells) + nbm[1]);
+                    gf[k][0][i] = __ldg(row_ptr(fx0, i, p.ncells));
+                    gf[k][1][i] = __ldg(row_ptr(fx1, i, p.ncells));
+                    gf[k][2][i] = __ldg(row_ptr(fy0, i, p.ncells));
+                    gf[k][3][i] = __ldg(row_ptr(fy1, i, p.ncells));
                 }
             }
         }

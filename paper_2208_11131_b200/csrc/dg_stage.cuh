@@ -696,6 +696,18 @@ struct TilePos {
             iz = cg / (p.nx * p.ny);
         }
     }
+    // the same for tile number t of the blocked order (persistent kernels; the mesh must qualify for tile_grid_blocked)
+    __device__ __forceinline__ TilePos(const DgStageArgs &p, int cl, int t) {
+        const int ntx = p.nx / C, nyy = 64 * (p.ny / 8);
+        const int bx = t % ntx, by = (t / ntx) % nyy, bz = t / (ntx * nyy);
+        const int r = by & 63;
+        iy = (by >> 6) * 8 + (r & 7);
+        iz = bz * 8 + (r >> 3);
+        cell0 = (iz * p.ny + iy) * p.nx + bx * C;
+        ix = bx * C + cl;
+        cg = cell0 + cl;
+        active = true;
+    }
     // periodic neighbours: lower (-1) / upper (+1) along each axis
     __device__ __forceinline__ int lower(const DgStageArgs &p, int a) const {
         if (a == 0) return cg + ((ix == 0) ? p.nx - 1 : -1);

@@ -28,6 +28,11 @@
 #ifndef DG_S2_MINB
 #define DG_S2_MINB 1
 #endif
+// persistent producer/consumer form of the 3D kernel: measured 2 % slower per step than one block per tile
+// (profiles/r2b_cfg4.md), off by default
+#ifndef DG_S2_PERSIST
+#define DG_S2_PERSIST 0
+#endif
 #ifndef DG_S2_UNROLL_E
 #define DG_S2_UNROLL_E 2
 #endif
@@ -61,28 +66,49 @@ struct Cfg2 {
     static constexpr int C = pick_c();
     static constexpr int kSmemBytes = (C * FP + extra_doubles(C)) * 8;
     static_assert(kSmemBytes <= kSmemMax, "stage kernel 2: per-cell footprint exceeds shared memory");
+    // persistent producer/consumer form (see the kernel): a second copy of U and of Wk; 3D only, when it fits and the
+    // consumer threads divide into the cells
+    static constexpr int kSmemPersist = kSmemBytes + (V * Np * C + C) * 8;
+    static constexpr bool kPersist = DG_S2_PERSIST && D == 3 && NT == 512 && kSmemPersist <= kSmemMax && ((NT - 128) % C == 0);
     static_assert(NT % C == 0, "threads per block must be a multiple of cells per block");
 };
 
 // PLAIN: the RK-stage form every time step uses (not rhs_only, full tensor basis, no SSPRK(5,4) auxiliary row): those
 // three switches become compile-time constants, which removes their selects from the combine loops.
-template <int D, int M, bool VISC, bool AV, bool PLAIN>
+//
+// PERSIST (3D, blocked tile order, ordinary stages without the Eq. 23 tail and without the limiter): one block per SM
+// walks the tiles b, b + gridDim.x, ...  Warps 12-15, which have no tile in phases A and G, become PRODUCERS: they run
+// phase A of the NEXT tile (global loads + x,y expansion) into a second copy of U while warps 0-11 (CONSUMERS, 24
+// threads per cell = one tile item each) run phases B-H of the current tile, so the DRAM round trip at the head of
+// every tile is hidden.  Hand-over through named barriers: FULL[b] (producers arrive, consumers wait), EMPTY[b]
+// (consumers arrive after their last read of U[b], producers wait), barrier 1 = the consumers' phase barrier.
+__device__ __forceinline__ void named_bar_sync(int id, int count) {
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory");
+}
+__device__ __forceinline__ void named_bar_arrive(int id, int count) {
+    asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(count) : "memory");
+}
+
+template <int D, int M, bool VISC, bool AV, bool PLAIN, bool PERSIST = false>
 __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_stage2_kernel(const DgStageArgs p) {
     using K = Cfg<D, M, VISC, AV>;
     using K2 = Cfg2<D, M, VISC, AV>;
-    constexpr int C = K2::C, NT = K2::NT, V = K::V, Vc = K::Vc, Np = K::Np, Nf = K::Nf;
+    constexpr int C = K2::C, NTB = K2::NT, V = K::V, Vc = K::Vc, Np = K::Np, Nf = K::Nf;
+    constexpr int NPROD = PERSIST ? 128 : 0;      // producer threads (the last four warps)
+    constexpr int NT = NTB - NPROD;               // threads that run the phases below (all of them unless PERSIST)
+    static_assert(!PERSIST || (D == 3 && PLAIN && NT % C == 0), "persistent form: 3D, plain stages");
     constexpr bool GRAD = K::GRAD;
     constexpr int MM = M * M;
     constexpr int kUnrollE = DG_S2_UNROLL_E, kUnrollB = DG_S2_UNROLL_B;
     constexpr int NTILE = Np / MM;               // m x m tiles per slot (m in 3D, 1 in 2D)
     using L = Lay<MM, Np, use_swizzle(M, C), 0>;
     extern __shared__ __align__(128) double smem[];
-    double *U = smem;                             // [V][Np][C]   modes -> nodal values -> projected N
-    double *GR = U + V * Np * C;                  // [D*Vc][Np][C] gradients -> fluxes (in place)
-    double *Wk = GR + D * Vc * Np * C;
-    double *red = Wk + C;
-    double *sens = red + 2 * (NT / 32);           // [4][NT/32][C] partial sensor sums (AV only)
-    double *sS = sens + (AV ? 4 * (NT / 32) * C : 0);   // weak-derivative matrix S for run-time row indices
+    double *U0 = smem;                            // [V][Np][C]   modes -> nodal values -> projected N  (x2 if PERSIST)
+    double *GR = U0 + (PERSIST ? 2 : 1) * V * Np * C;   // [D*Vc][Np][C] gradients -> fluxes (in place)
+    double *Wk0 = GR + D * Vc * Np * C;           // [C] (x2 if PERSIST)
+    double *red = Wk0 + (PERSIST ? 2 : 1) * C;
+    double *sens = red + 2 * (NTB / 32);          // [4][NTB/32][C] partial sensor sums (AV only)
+    double *sS = sens + (AV ? 4 * (NTB / 32) * C : 0);   // weak-derivative matrix S for run-time row indices
     double *limsc = sS + M * M + 2;                     // limiter scratch (fused form)
     double *ldev = limsc + LimScratch<D, C>::kDoubles;  // [Vc][C] sum_{l>0} |w_l| max|phi_l| of the new state
     const bool lim = (p.limiter != 0);
@@ -99,15 +125,56 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
     const double cdtp = cdt * pref;
     const bool sens_stage = p.do_sensor != 0;
     if (tid < MM) sS[tid] = c_tab.S[(tid / M) * 8 + tid % M];
-    {
-        const TilePos<D, C> pos(p, cl);
+    auto cbar = [&]() {                           // barrier between the phases
+        if (PERSIST)
+            named_bar_sync(1, NT);
+        else
+            __syncthreads();
+    };
+    if (PERSIST) __syncthreads();                 // sS
+    if (PERSIST && tid >= NT) {
+        // ---- producers: phase A of every tile of this block, one tile ahead of the consumers ----
+        const int ptid = tid - NT, pcl = ptid % C;
+        int itile = 0;
+        for (int t = blockIdx.x; t < p.ntiles; t += gridDim.x, ++itile) {
+            const int b = itile & 1;
+            double *U = U0 + b * V * Np * C;
+            if (itile >= 2) named_bar_sync(4 + b, NTB);          // consumers are done with this copy of U
+            const TilePos<D, C> pos(p, pcl, t);
+            if (AV && ptid < C) {
+                const double S = p.sens_prev[pos.cg];
+                const double G = p.sens_prev[p.ncells + pos.cg];
+                (Wk0 + b * C)[ptid] = (S > p.s_onset) ? p.f_w * fmax(0.0, G) : 0.0;
+            }
+            for (int it = ptid; it < V * NTILE * C; it += NPROD) {
+                const int g = it / C;
+                const int v = g / NTILE, lz = g % NTILE;
+                double tl[MM];
+                const double *src = p.w_prev + (size_t)(lz * MM * V + v) * p.ncells + pos.cg;
+#pragma unroll
+                for (int q = 0; q < MM; ++q) tl[q] = __ldg(row_ptr(src, q * V, p.ncells));
+                tile_x<DG_SEL_V, M>(tl);
+                tile_y<DG_SEL_V, M>(tl);
+                tile_store<M, C, L>(U, g, pcl, tl);
+            }
+            __threadfence_block();
+            named_bar_arrive(2 + b, NTB);                        // this copy of U is full
+        }
+        return;
+    }
+    int itile = 0;
+    for (int tl_ = PERSIST ? (int)blockIdx.x : 0; PERSIST ? (tl_ < p.ntiles) : (itile < 1); tl_ += gridDim.x, ++itile) {
+        double *U = U0 + (PERSIST ? (itile & 1) * V * Np * C : 0);
+        double *Wk = Wk0 + (PERSIST ? (itile & 1) * C : 0);
+        const TilePos<D, C> pos = PERSIST ? TilePos<D, C>(p, cl, tl_) : TilePos<D, C>(p, cl);
         const int cell0 = pos.cell0;
         const int cg = pos.cg;
         const bool active = pos.active;
         int nbm[D];                               // lower neighbour along each axis (periodic wrap)
 #pragma unroll
         for (int a = 0; a < D; ++a) nbm[a] = pos.lower(p, a);
-        if (AV && tid < C) {
+        if (PERSIST) named_bar_sync(2 + (itile & 1), NTB);   // phase A of this tile has landed in U
+        if (!PERSIST && AV && tid < C) {
             // wiggle source of Eq. 45 from the previous step's sensor (readings A14, A15)
             const int c = min(cell0 + tid, p.ncells - 1);
             const double S = p.sens_prev[c];
@@ -116,7 +183,7 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
         }
 
         // ---- A: own modes, global -> register tile; expansion along x and y (Eq. 21) ----
-        for (int it = tid; it < V * NTILE * C; it += NT) {
+        for (int it = tid; !PERSIST && it < V * NTILE * C; it += NT) {
             const int g = it / C;                 // v*NTILE + lz
             const int v = g / NTILE, lz = g % NTILE;
             double t[MM];
@@ -136,7 +203,7 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
                 tile_store<M, C, L>(GR, Vc * NTILE + g, cl, t);
             }
         }
-        __syncthreads();
+        cbar();
         if (D == 3) {
             // ---- B: expansion along z, z derivative ----
             constexpr int NKB = (V * MM * C + NT - 1) / NT;
@@ -159,7 +226,7 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
                     for (int j = 0; j < M; ++j) GR[L::at2(2 * Vc + v, q + j * MM) * C + cl] = gz[j];
                 }
             }
-            __syncthreads();
+            cbar();
             if (GRAD) {
                 // ---- D: x and y derivatives of the nodal values, one tile load for both ----
                 for (int it = tid; it < Vc * NTILE * C; it += NT) {
@@ -173,7 +240,7 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
                     tile_y<DG_SEL_DHAT, M>(t);
                     tile_store<M, C, L>(GR, Vc * NTILE + g, cl, t);
                 }
-                __syncthreads();
+                cbar();
             }
         }
         {
@@ -296,10 +363,10 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
                 }
             }
         }
-        __syncthreads();
+        cbar();
         if (AV && p.do_sensor && tid == 0) {
             double a = red[0];
-            for (int i = 1; i < NT / 32; ++i) a = fmax(a, red[i]);
+            for (int i = 1; i < NT / 32; ++i) a = fmax(a, red[i]);   // NT / 32 = the warps that ran phase E
             atomic_max_nonneg(&p.maxbits[2], a);
         }
 
@@ -396,10 +463,14 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
             // every global input of this thread's items (u^n, u^(i-1), the two z-face fluxes) is requested before the
             // barrier, so that one memory round trip covers them all and overlaps the wait for the other warps
             constexpr int NKH = (V * MM * C + NT - 1) / NT;
-            double hwn[NKH][M], hwp[NKH][M], hfz[NKH][2];
+            // items per load batch: all of them, or two at a time when a thread has four (persistent form: registers)
+            constexpr int HP = (PERSIST && NKH % 2 == 0) ? 2 : NKH;
 #pragma unroll
-            for (int k = 0; k < NKH; ++k) {
-                const int r = (tid + k * NT) / C;
+            for (int k0 = 0; k0 < NKH; k0 += HP) {
+            double hwn[HP][M], hwp[HP][M], hfz[HP][2];
+#pragma unroll
+            for (int k = 0; k < HP; ++k) {
+                const int r = (tid + (k0 + k) * NT) / C;
                 const int q = r % MM, v = r / MM;     // q = ly*M + lx
                 hfz[k][0] = hfz[k][1] = 0.0;
 #pragma unroll
@@ -419,10 +490,10 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
                     }
                 }
             }
-            __syncthreads();
+            if (k0 == 0) cbar();
 #pragma unroll
-            for (int k = 0; k < NKH; ++k) {
-                const int r = (tid + k * NT) / C;
+            for (int k = 0; k < HP; ++k) {
+                const int r = (tid + (k0 + k) * NT) / C;
                 if (r >= V * MM) break;
                 const int q = r % MM, v = r / MM;
                 double *bo = p.w_out + (size_t)(q * V + v) * p.ncells + cg;
@@ -469,6 +540,7 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
                 }
                 if (lim && v < Vc) atomicAdd(&ldev[v * C + cl], hdev);
             }
+            }   // load batches of phase H
         }
         if (AV && p.do_sensor) {
             // lanes of a warp that share a cell (lane = cl + C*j), then one partial per warp and cell in `sens`
@@ -486,7 +558,7 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
                 sens[(2 * NW + tid / 32) * C + cl] = dA;
                 sens[(3 * NW + tid / 32) * C + cl] = dB;
             }
-            __syncthreads();
+            cbar();
             if (tid < C && cell0 + tid < p.ncells) {
                 double s[4] = {0.0, 0.0, 0.0, 0.0};
                 for (int k = 0; k < NW; ++k)
@@ -502,7 +574,10 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
             p.sens_prev[c] = p.sens_new[c];
             p.sens_prev[p.ncells + c] = p.sens_new[p.ncells + c];
         }
-        if (lim) {
+        if (PERSIST) {
+            // last read of this copy of U (phase H) is done: hand it back to the producers if they will need it again
+            if (tl_ + 2 * (int)gridDim.x < p.ntiles) named_bar_arrive(4 + (itile & 1), NTB);
+        } else if (lim) {
             // ---- positivity limiter on the stage output (Eq. 47; readings L1-L6), fused: the new
             //      modes of the d+2 conserved fields are still in U, the face point values go to the (now free) flux
             //      array; cells with F != 1 re-read their freshly written rows (L2) and scale every mode but the mean ----

@@ -29,6 +29,12 @@ cudaError_t configure() {
                                  cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  DG_NS::Cfg2<DG_DIM, DG_M, VISC, AV>::kSmemBytes);
         if (e != cudaSuccess) return e;
+        if constexpr (DG_NS::Cfg2<DG_DIM, DG_M, VISC, AV>::kPersist) {
+            e = cudaFuncSetAttribute(DG_NS::dg_stage2_kernel<DG_DIM, DG_M, VISC, AV, true, true>,
+                                     cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     DG_NS::Cfg2<DG_DIM, DG_M, VISC, AV>::kSmemPersist);
+            if (e != cudaSuccess) return e;
+        }
     }
     e = cudaFuncSetAttribute(DG_NS::dg_face_kernel<DG_DIM, DG_M, VISC, AV>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              DG_NS::FaceCfg<DG_DIM, DG_M, VISC, AV>::kSmemBytes);
@@ -61,7 +67,24 @@ cudaError_t launch(const DgStageArgs &a, cudaStream_t st, int wavespeed_only) {
             // register-tile configurations (2 <= m <= 5): second-generation stage kernel (dg_stage2.cuh)
             using K2 = DG_NS::Cfg2<DG_DIM, DG_M, VISC, AV>;
             const dim3 grid2 = DG_NS::tile_grid<DG_DIM, K2::C>(a.ncells, a.nx, a.ny, a.nz);
-            if (!a.rhs_only && !a.total_degree && a.w_aux == nullptr)
+            const bool plain = !a.rhs_only && !a.total_degree && a.w_aux == nullptr;
+            if constexpr (K2::kPersist) {
+                if (plain && !a.do_wavespeed && !a.limiter && grid2.y > 1) {
+                    // persistent form: one block per SM, producer warps load the next tile (dg_stage2.cuh)
+                    static int sms = 0;
+                    if (!sms) {
+                        int dev = 0;
+                        cudaGetDevice(&dev);
+                        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+                    }
+                    DgStageArgs b = a;
+                    b.ntiles = (int)(grid2.x * grid2.y * grid2.z);
+                    const int nb = b.ntiles < sms ? b.ntiles : sms;
+                    DG_NS::dg_stage2_kernel<DG_DIM, DG_M, VISC, AV, true, true><<<nb, K2::NT, K2::kSmemPersist, st>>>(b);
+                    return cudaGetLastError();
+                }
+            }
+            if (plain)
                 DG_NS::dg_stage2_kernel<DG_DIM, DG_M, VISC, AV, true><<<grid2, K2::NT, K2::kSmemBytes, st>>>(a);
             else
                 DG_NS::dg_stage2_kernel<DG_DIM, DG_M, VISC, AV, false><<<grid2, K2::NT, K2::kSmemBytes, st>>>(a);

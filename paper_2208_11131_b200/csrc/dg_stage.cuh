@@ -69,6 +69,9 @@
 #ifndef DG_FACE_DIRECT
 #define DG_FACE_DIRECT 1
 #endif
+#ifndef DG_FACE_DIRECT_CMAX
+#define DG_FACE_DIRECT_CMAX 16
+#endif
 #ifndef DG_FACE_DIRECT_MINB
 #define DG_FACE_DIRECT_MINB 3
 #endif
@@ -837,7 +840,7 @@ struct FaceCfg {
     static constexpr bool DIRECT = DG_FACE_DIRECT && ((K::BLK && D == 3) || GLay<D, M>::B > 0);
     static constexpr int FP = (DIRECT ? 0 : K::V * K::Np) + K::NQ * K::Nf;   // doubles per cell: [own modes +] one face
     static constexpr int MINB = BIG ? 1 : (DIRECT ? DG_FACE_DIRECT_MINB : DG_FACE_MINB);   // resident blocks per SM (register cap)
-    static constexpr int CMAX = DIRECT ? 16 : 32;
+    static constexpr int CMAX = DIRECT ? DG_FACE_DIRECT_CMAX : 32;
     static constexpr int pick_c() {
         int c = CMAX;
         while (c > 1 && c * FP * 8 > (227 * 1024) / MINB - 2048) c >>= 1;   // MINB resident blocks per SM

@@ -227,7 +227,7 @@ __device__ __forceinline__ void apply1d(const double *in, double *out) {
     if (DG_EVEN_ODD && M >= 2 && SEL == DG_SEL_V) {
 #pragma unroll
         for (int j = 0; j < H; ++j) {
-            double e = c_tab.V[j * 8] * in[0];
+            double e = in[0];                       // P_0 = 1 exactly (normalised Legendre): no multiplication
 #pragma unroll
             for (int l = 2; l < M; l += 2) e = fma(c_tab.V[j * 8 + l], in[l], e);
             double o = c_tab.V[j * 8 + 1] * in[1];
@@ -237,7 +237,7 @@ __device__ __forceinline__ void apply1d(const double *in, double *out) {
             out[M - 1 - j] = e - o;
         }
         if (M % 2) {
-            double e = c_tab.V[H * 8] * in[0];
+            double e = in[0];
 #pragma unroll
             for (int l = 2; l < M; l += 2) e = fma(c_tab.V[H * 8 + l], in[l], e);
             out[H] = e;

@@ -69,6 +69,9 @@
 #ifndef DG_FACE_DIRECT
 #define DG_FACE_DIRECT 1
 #endif
+#ifndef DG_FACE_BIG_MINB
+#define DG_FACE_BIG_MINB 1
+#endif
 #ifndef DG_FACE_DIRECT_CMAX
 #define DG_FACE_DIRECT_CMAX 16
 #endif
@@ -839,7 +842,7 @@ struct FaceCfg {
     // not wait for it before the first axis, and only the face scratch remains (more cells or blocks per SM)
     static constexpr bool DIRECT = DG_FACE_DIRECT && ((K::BLK && D == 3) || GLay<D, M>::B > 0);
     static constexpr int FP = (DIRECT ? 0 : K::V * K::Np) + K::NQ * K::Nf;   // doubles per cell: [own modes +] one face
-    static constexpr int MINB = BIG ? 1 : (DIRECT ? DG_FACE_DIRECT_MINB : DG_FACE_MINB);   // resident blocks per SM (register cap)
+    static constexpr int MINB = BIG ? DG_FACE_BIG_MINB : (DIRECT ? DG_FACE_DIRECT_MINB : DG_FACE_MINB);   // resident blocks per SM (register cap)
     static constexpr int CMAX = DIRECT ? DG_FACE_DIRECT_CMAX : 32;
     static constexpr int pick_c() {
         int c = CMAX;

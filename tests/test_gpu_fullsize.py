@@ -141,7 +141,7 @@ def test_cfg5_full_length_exact_solution(degree):
         degree, err, drift))
 
 
-@pytest.mark.parametrize("degree", [1, 2, 3])
+@pytest.mark.parametrize("degree", [1, 2, 3, 5, 7])     # 5, 7: the block layout (4 and 2 cells per block)
 def test_cfg5_full_size_sampled_state_after_one_step(degree):
     wl = wk.config(5, degree=degree)
     d, Vc, M, N = wl.dim, wl.dim + 2, wl.modes, wl.ncells

@@ -103,7 +103,36 @@ def test_cfg4_full_size_50_steps():
     g = make_gpu(wl)
     g.set_state(host)
     t0 = g.conserved_totals()
-    g.step(50)
+    # one RK3 step at full size in the bench launch configuration, compared on sampled cells with the oracle run on the
+    # periodic 7x7x7 patch around each cell (exact: three stages reach three cells)
+    g.step(1)
+    _, dt = g.get_time()
+    d, Vc, M, N = wl.dim, wl.dim + 2, wl.modes, wl.ncells
+    w1 = g.get_state().reshape(M, Vc, N)
+    a1 = g.get_alpha().reshape(M, N)
+    nx, ny, nz = wl.ncell
+    wv = host.numpy().reshape(M, Vc, nz, ny, nx)
+    sub = replace(wl, ncell=(7, 7, 7))
+    worst = 0.0
+    for (ix, iy, iz) in [(0, 0, 0), (127, 127, 127), (127, 0, 64), (5, 120, 1), (64, 64, 64)]:
+        zi = [(iz + k) % nz for k in range(-3, 4)]
+        yi = [(iy + k) % ny for k in range(-3, 4)]
+        xi = [(ix + k) % nx for k in range(-3, 4)]
+        o = make_oracle(sub, fixed_dt=dt)
+        o.set_state(np.ascontiguousarray(wv[:, :, zi][:, :, :, yi][:, :, :, :, xi]).ravel())
+        assert o.step(1) == 0
+        centre = (3 * 7 + 3) * 7 + 3
+        ref = o.get_state().reshape(M, Vc, 343)
+        cell = (iz * ny + iy) * nx + ix
+        scale = np.max(np.abs(ref[0]), axis=1)
+        scale[1:1 + d] = np.max(scale[1:1 + d]) + np.max(np.abs(ref[0, 0]))
+        err = np.max(np.abs(w1[:, :, cell] - ref[:, :, centre]) / scale[None, :])
+        aerr = np.max(np.abs(a1[:, cell] - o.get_alpha().reshape(M, 343)[:, centre]))
+        worst = max(worst, err)
+        assert err <= TOL_1 and aerr <= 1e-9, ((ix, iy, iz), err, aerr)
+    del w1, a1
+    _report("cfg4 FULL SIZE 128^3: state after 1 step on sampled cells, worst %.3e" % worst)
+    g.step(49)
     d = g.diagnostics()
     assert d["steps"] == 50 and d["unphysical"] == 0
     drift = _drift(g.conserved_totals(), t0, wl)

@@ -69,6 +69,14 @@
 #ifndef DG_FACE_DIRECT
 #define DG_FACE_DIRECT 1
 #endif
+// row rotation of the pencil-sweep layouts: only where the row index arithmetic is shifts (m = 8); at m = 6 the
+// divisions by 6 cost more than the bank conflicts they avoid (stage kernel 2.80 -> 2.50 ms without it)
+#ifndef DG_ROT_NONPOW2
+#define DG_ROT_NONPOW2 0
+#endif
+#ifndef DG_ROT_ENABLE
+#define DG_ROT_ENABLE 1
+#endif
 #ifndef DG_FACE_BIG_MINB
 #define DG_FACE_BIG_MINB 1
 #endif
@@ -207,7 +215,9 @@ struct Lay {
 };
 __host__ __device__ constexpr bool use_swizzle(int M, int C) { return (M % 2 == 0) && (C == 8); }
 // rotation for the pencil-sweep path (m x m tiles not in registers), few cells per block, even m
-__host__ __device__ constexpr int use_rot(int M, int C, bool BLK) { return (!BLK && C < 8 && M % 2 == 0 && M > 1) ? M : 0; }
+__host__ __device__ constexpr int use_rot(int M, int C, bool BLK) {
+    return (DG_ROT_ENABLE && !BLK && C < 8 && M % 2 == 0 && M > 1 && (DG_ROT_NONPOW2 || (M & (M - 1)) == 0)) ? M : 0;
+}
 
 template <int SEL>
 __device__ __forceinline__ double mat(int idx) {

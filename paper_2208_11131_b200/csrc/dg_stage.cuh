@@ -1188,12 +1188,20 @@ __global__ void __launch_bounds__((Cfg<D, M, VISC, AV>::NT), DG_STAGE_MINB) dg_s
     const int cg = min(cell0 + cl, p.ncells - 1);
     int nbm[D];                                  // lower neighbour along each axis (periodic wrap)
     {
-        const int ix = cg % p.nx;
-        const int iy = (cg / p.nx) % p.ny;
-        const int iz = cg / (p.nx * p.ny);
-        nbm[0] = cg + ((ix == 0) ? p.nx - 1 : -1);
-        nbm[1] = cg + ((iy == 0) ? (p.ny - 1) * p.nx : -p.nx);
-        if (D == 3) nbm[D - 1] = cg + ((iz == 0) ? (p.nz - 1) * p.nx * p.ny : -p.nx * p.ny);
+        // the integer divisions of cell -> (ix, iy, iz) once per cell of the block, not once per thread
+        __shared__ int s_nbm[D][32];
+        if (tid < C) {
+            const int c = min(cell0 + tid, p.ncells - 1);
+            const int ix = c % p.nx;
+            const int iy = (c / p.nx) % p.ny;
+            const int iz = c / (p.nx * p.ny);
+            s_nbm[0][tid] = c + ((ix == 0) ? p.nx - 1 : -1);
+            s_nbm[1][tid] = c + ((iy == 0) ? (p.ny - 1) * p.nx : -p.nx);
+            if (D == 3) s_nbm[D - 1][tid] = c + ((iz == 0) ? (p.nz - 1) * p.nx * p.ny : -p.nx * p.ny);
+        }
+        __syncthreads();
+#pragma unroll
+        for (int a = 0; a < D; ++a) nbm[a] = s_nbm[a][cl];
     }
     // ---- front loads, all in flight before the first barrier: face fluxes of the 2D faces, own modes ----
     constexpr int NFL = Vc * K::Nf;                       // flux values per cell and axis

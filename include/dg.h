@@ -184,6 +184,47 @@ int dg_launch_count(dg_solver *s, long long *count);
  * `iters` iterations on every SM (roofline denominator for the ALU-bound configs). */
 int dg_measure_fp64_peak(int iters, double *flops_per_s, void *cuda_stream);
 
+/* Conserved totals for callers that must not allocate device memory.
+ *
+ * Who this is for: code that runs where every byte of the GPU is already spoken for or where an allocation is simply
+ * not allowed at that point -- an in-situ diagnostics hook called from inside somebody else's time loop on a device
+ * the simulation has filled, a plug-in living inside a framework whose memory pool owns the whole card (a raw
+ * cudaMalloc beside the pool fails or fragments it), a job started under a hard per-process memory cap, or a
+ * latency-bound monitoring thread that cannot afford the device-wide stall cudaMalloc / cudaFree imply.  Such callers
+ * cannot create a dg_solver (dg_init allocates, dg_init_workspace needs a workspace somebody allocated) just to ask
+ * "how much mass, momentum and energy is in this state?".
+ *
+ * What it computes: the same quantity as dg_conserved_totals -- cell_volume * sum over cells of the mode-0 weight
+ * (the cell mean) of each of the first `nvars` variables -- by a compensated, fixed-shape and
+ * therefore run-to-run reproducible reduction (4096 cells per block, block partials combined in block order).
+ *
+ *   w            DEVICE pointer (on the current device) to a modal state in the layout at the top of this file; only
+ *                the rows of mode 0 are read, i.e. w[var*ncells + cell] for var < nvars.  Caller-owned, read only.
+ *   nvars        how many leading variables to total, 1 .. DG_NOALLOC_MAX_VARS (dim+2, or dim+3 with the tracer row).
+ *   ncells       cells of the mesh, 1 .. DG_NOALLOC_MAX_CELLS.  Larger meshes are refused with DG_EINVAL and a text
+ *                that names the limit; nothing is launched in that case.
+ *   cell_volume  h^dim.
+ *   totals       `nvars` doubles, HOST or DEVICE pointer, caller-owned.  DEVICE: the result is written in stream
+ *                order and the call returns without waiting.  HOST: the call copies the result out and waits for
+ *                `cuda_stream` before it returns.
+ *   cuda_stream  cudaStream_t passed as void* (NULL = default stream).
+ *
+ * Scratch memory: the block partials live in ONE array compiled into the library (static __device__, 131 136 bytes =
+ * (2*8*1024 + 8) doubles).  Every GPU that loads the library carries that array until the process exits, whether or
+ * not this function is ever called.  The function itself calls no cudaMalloc / cudaFree / allocating library routine.
+ *   - First call on each device: looks up the device address of that array (cudaGetSymbolAddress, with the calling
+ *     thread's current device) and remembers it; this may make the CUDA runtime load the library's kernels on that
+ *     device.  Make this first call outside any stream capture and with the device you mean to use current.
+ *   - All calls on a device share the array and it keeps whatever the previous call left.  Nothing in it has to start
+ *     at zero: each call first writes every slot it later reads.  But two calls that overlap on the GPU (different
+ *     streams, or two host threads) race on it and return garbage -- serialise them on one stream.
+ * Errors: DG_EINVAL (NULL pointer, nvars / ncells out of range, w not device memory of the current device),
+ * DG_ECUDA (no device, or a CUDA call failed). */
+#define DG_NOALLOC_MAX_CELLS 4194304   /* 2^22 cells = 1024 blocks of 4096 cells; a 128^3 mesh is half of this */
+#define DG_NOALLOC_MAX_VARS  8
+int dg_totals_noalloc(const double *w, int nvars, long long ncells, double cell_volume, double *totals,
+                      void *cuda_stream);
+
 /* Free all device state.  NULL is allowed. */
 int dg_free(dg_solver *s);
 

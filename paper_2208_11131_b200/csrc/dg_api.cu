@@ -5,6 +5,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 #include "../../include/dg.h"
@@ -511,6 +512,109 @@ int from_internal(dg_solver *s, double *ext, const double *W, int var0, int nv) 
 
 }  // namespace
 
+// ---- dg_totals_noalloc: conserved totals without any device allocation (include/dg.h) ---------------------
+//
+// The solver path (dg_totals_kernel) parks its per-variable results in the solver's workspace, which somebody had to
+// allocate.  Callers that are not allowed to allocate -- a diagnostics hook on a GPU the host simulation has filled,
+// code inside a framework whose pool owns the card, a process under a fixed memory cap, a thread that must not
+// trigger the device-wide stall of cudaMalloc -- get the same sums from the array below instead.  It is part of the
+// library image: each GPU that loads the library holds these 131 136 bytes until the process ends.
+//
+// Layout: [ (var * kNaMaxBlocks + block) * 2 + {0: sum, 1: compensation} ]  block partials of the first pass,
+//         [ kNaPartials + var ]                                              finished totals when `totals` is host memory.
+// In host code the identifier dg_noalloc_scratch is only a handle for the runtime, not a device address: the kernels
+// get the pointer cudaGetSymbolAddress returns for the current device (noalloc_scratch_for_current_device).
+constexpr int kNaChunk = 4096;                                      // cells per block of the first pass
+constexpr int kNaThreads = 256;                                     // 16 cells per thread
+constexpr int kNaMaxBlocks = DG_NOALLOC_MAX_CELLS / kNaChunk;       // 1024 = threads of the second pass
+constexpr size_t kNaPartials = (size_t)2 * DG_NOALLOC_MAX_VARS * kNaMaxBlocks;
+static_assert(kNaMaxBlocks == 1024 && DG_NOALLOC_MAX_CELLS % kNaChunk == 0, "second pass: one thread per block partial");
+
+static __device__ __align__(256) double dg_noalloc_scratch[kNaPartials + DG_NOALLOC_MAX_VARS];
+
+namespace {
+
+// Neumaier step: (s, c) += x
+__device__ inline void na_add(double &s, double &c, double x) {
+    const double t = s + x;
+    c += (fabs(s) >= fabs(x)) ? ((s - t) + x) : ((x - t) + s);
+    s = t;
+}
+
+// fixed-shape tree over the (sum, compensation) pairs of a block; result in ss[0], sc[0]
+template <int NT>
+__device__ inline void na_block_tree(double *ss, double *sc) {
+    __syncthreads();
+    for (int o = NT / 2; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) {
+            const double a = ss[threadIdx.x], b = ss[threadIdx.x + o];
+            const double t = a + b;
+            const double e = (fabs(a) >= fabs(b)) ? ((a - t) + b) : ((b - t) + a);
+            ss[threadIdx.x] = t;
+            sc[threadIdx.x] += sc[threadIdx.x + o] + e;
+        }
+        __syncthreads();
+    }
+}
+
+// pass 1: block (b, v) sums cells [b*4096, (b+1)*4096) of the mode-0 row of variable v into its scratch slot
+__global__ void __launch_bounds__(kNaThreads) dg_noalloc_partial_kernel(const double *w, long long ncells, double *scratch) {
+    __shared__ double ss[kNaThreads], sc[kNaThreads];
+    const int v = blockIdx.y;
+    const double *row = w + (size_t)v * (size_t)ncells;
+    const long long base = (long long)blockIdx.x * kNaChunk;
+    double s = 0.0, c = 0.0;
+#pragma unroll 4
+    for (int k = 0; k < kNaChunk / kNaThreads; ++k) {
+        const long long i = base + k * kNaThreads + threadIdx.x;
+        if (i < ncells) na_add(s, c, row[i]);
+    }
+    ss[threadIdx.x] = s;
+    sc[threadIdx.x] = c;
+    na_block_tree<kNaThreads>(ss, sc);
+    if (threadIdx.x == 0) {
+        double *slot = scratch + ((size_t)v * kNaMaxBlocks + blockIdx.x) * 2;
+        slot[0] = ss[0];
+        slot[1] = sc[0];
+    }
+}
+
+// pass 2: block v combines the nblk partials of variable v (slots beyond nblk hold an older call's data: not read)
+__global__ void __launch_bounds__(kNaMaxBlocks) dg_noalloc_finish_kernel(const double *scratch, int nblk, double vol,
+                                                                        double *out) {
+    __shared__ double ss[kNaMaxBlocks], sc[kNaMaxBlocks];
+    const int v = blockIdx.x;
+    const bool live = (int)threadIdx.x < nblk;
+    const double *slot = scratch + ((size_t)v * kNaMaxBlocks + threadIdx.x) * 2;
+    ss[threadIdx.x] = live ? slot[0] : 0.0;
+    sc[threadIdx.x] = live ? slot[1] : 0.0;
+    na_block_tree<kNaMaxBlocks>(ss, sc);
+    if (threadIdx.x == 0) out[v] = vol * (ss[0] + sc[0]);
+}
+
+// Device address of dg_noalloc_scratch on the calling thread's current device; looked up once per device.
+constexpr int kNaMaxDevices = 64;
+double *g_na_ptr[kNaMaxDevices] = {};
+std::mutex g_na_mutex;
+
+int noalloc_scratch_for_current_device(int dev, double **ptr) {
+    if (dev < 0 || dev >= kNaMaxDevices) return fail(DG_ECUDA, "dg_totals_noalloc: device ordinal beyond 63%s");
+    std::lock_guard<std::mutex> lock(g_na_mutex);
+    if (!g_na_ptr[dev]) {
+        void *p = nullptr;
+        cudaError_t e = cudaGetSymbolAddress(&p, dg_noalloc_scratch);
+        if (e != cudaSuccess || !p) {
+            cudaGetLastError();
+            return fail(DG_ECUDA, "cudaGetSymbolAddress(dg_noalloc_scratch): %s", cudaGetErrorString(e));
+        }
+        g_na_ptr[dev] = (double *)p;
+    }
+    *ptr = g_na_ptr[dev];
+    return DG_OK;
+}
+
+}  // namespace
+
 extern "C" {
 
 int dg_default_options(dg_options *opt) {
@@ -929,6 +1033,58 @@ int dg_measure_fp64_peak(int iters, double *flops_per_s, void *cuda_stream) {
     if (e != cudaSuccess) return fail(DG_ECUDA, "dg_measure_fp64_peak: %s", cudaGetErrorString(e));
     const double flops = 2.0 * 64.0 * (double)iters * 256.0 * (double)blocks;
     *flops_per_s = flops / (ms * 1e-3);
+    return DG_OK;
+}
+
+int dg_totals_noalloc(const double *w, int nvars, long long ncells, double cell_volume, double *totals,
+                      void *cuda_stream) {
+    if (!w || !totals) return fail(DG_EINVAL, "dg_totals_noalloc: NULL argument%s");
+    if (nvars < 1 || nvars > DG_NOALLOC_MAX_VARS) {
+        std::snprintf(g_err, sizeof(g_err), "dg_totals_noalloc: nvars = %d is outside 1..%d (DG_NOALLOC_MAX_VARS)", nvars,
+                      DG_NOALLOC_MAX_VARS);
+        return DG_EINVAL;
+    }
+    if (ncells < 1 || ncells > (long long)DG_NOALLOC_MAX_CELLS) {
+        std::snprintf(g_err, sizeof(g_err),
+                      "dg_totals_noalloc: ncells = %lld is outside 1..%d (DG_NOALLOC_MAX_CELLS): the scratch array built "
+                      "into the library has one slot per 4096 cells and cannot grow; use dg_conserved_totals of a solver",
+                      ncells, DG_NOALLOC_MAX_CELLS);
+        return DG_EINVAL;
+    }
+    if (!std::isfinite(cell_volume)) return fail(DG_EINVAL, "dg_totals_noalloc: cell_volume must be finite%s");
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) {
+        cudaGetLastError();
+        return fail(DG_ECUDA, "dg_totals_noalloc: no CUDA device: this library has no CPU path%s");
+    }
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, w) != cudaSuccess ||
+        (at.type != cudaMemoryTypeDevice && at.type != cudaMemoryTypeManaged)) {
+        cudaGetLastError();
+        return fail(DG_EINVAL, "dg_totals_noalloc: w must be a device pointer%s");
+    }
+    if (at.type == cudaMemoryTypeDevice && at.device != dev)
+        return fail(DG_EINVAL, "dg_totals_noalloc: w lives on another device than the current one%s");
+    bool out_on_device = false;
+    if (cudaPointerGetAttributes(&at, totals) == cudaSuccess &&
+        (at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged))
+        out_on_device = true;
+    else
+        cudaGetLastError();
+    double *scratch = nullptr;
+    int rc = noalloc_scratch_for_current_device(dev, &scratch);   // first call on this device: symbol look-up
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int nblk = (int)((ncells + kNaChunk - 1) / kNaChunk);
+    double *result = out_on_device ? totals : scratch + kNaPartials;
+    dg_noalloc_partial_kernel<<<dim3(nblk, nvars), kNaThreads, 0, st>>>(w, ncells, scratch);
+    CU(cudaGetLastError());
+    dg_noalloc_finish_kernel<<<nvars, kNaMaxBlocks, 0, st>>>(scratch, nblk, cell_volume, result);
+    CU(cudaGetLastError());
+    if (!out_on_device) {
+        CU(cudaMemcpyAsync(totals, result, (size_t)nvars * sizeof(double), cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+    }
     return DG_OK;
 }
 

@@ -73,6 +73,7 @@ SYMBOLS = {
     "dg_apply_limiter": (C.c_int, [_P]),
     "dg_launch_count": (C.c_int, [_P, C.POINTER(C.c_longlong)]),
     "dg_measure_fp64_peak": (C.c_int, [C.c_int, C.POINTER(C.c_double), _P]),
+    "dg_totals_noalloc": (C.c_int, [_P, C.c_int, C.c_longlong, C.c_double, _P, _P]),
     "dg_free": (C.c_int, [_P]),
     "dg_last_error": (C.c_char_p, []),
 }
@@ -287,6 +288,34 @@ def measure_fp64_peak(iters=4096, cuda_stream=0):
     v = C.c_double()
     _check(load_library().dg_measure_fp64_peak(iters, C.byref(v), cuda_stream))
     return v.value
+
+
+NOALLOC_MAX_CELLS, NOALLOC_MAX_VARS = 4194304, 8     # DG_NOALLOC_MAX_CELLS / DG_NOALLOC_MAX_VARS of include/dg.h
+
+
+def totals_noalloc(w, nvars, ncells, cell_volume, out=None, cuda_stream=None):
+    """dg_totals_noalloc: cell_volume * sum over cells of the cell means of the first `nvars` variables of the modal
+    state `w`, for callers that may not allocate device memory (a hook on a GPU somebody else has filled, code inside
+    a pool that owns the card, a process under a memory cap): the library's built-in scratch array is used, no
+    solver handle and no workspace are needed, and meshes beyond NOALLOC_MAX_CELLS are refused.
+
+    `w` is a cuda float64 tensor in the C-ABI state layout (at least nvars*ncells elements; only mode 0 is read);
+    `out` (nvars float64 values) may be a numpy array, a host tensor or a cuda tensor -- with a cuda tensor nothing
+    is waited for, and with out=None a new numpy array is returned.  The first call on a device should happen
+    outside stream capture; calls that overlap on the GPU share the scratch array and race (see include/dg.h)."""
+    pw, nw, _keep = _buf(w)
+    if nw < int(nvars) * int(ncells):
+        raise ValueError("w holds fewer than nvars*ncells values")
+    if out is None:
+        out = np.empty(int(nvars))
+    po, no, _keep2 = _buf(out)
+    if no < int(nvars):
+        raise ValueError("out holds fewer than nvars values")
+    if cuda_stream is None:
+        import torch
+        cuda_stream = torch.cuda.current_stream().cuda_stream if torch.cuda.is_available() else 0
+    _check(load_library().dg_totals_noalloc(pw, int(nvars), int(ncells), float(cell_volume), po, cuda_stream))
+    return out
 
 
 def from_workload(wl, **opt_kw) -> Solver:

@@ -39,6 +39,14 @@ def _drift(t1, t0, wl):
     return np.max(np.abs(t1 - t0) / scale)
 
 
+def _oracle_wave_speeds(o, wflat, wl, cells):
+    """Eq. 23 inputs of the oracle, o.wave_speeds, over the cells `cells` (an index array or slice into
+    the cell axis) of a full-size state in the C-ABI layout; `o` is any oracle of the same order and physics."""
+    M, Vc = wl.modes, wl.dim + 2
+    w = np.asarray(wflat).reshape(M, Vc, wl.ncells)[:, :, cells]
+    return o.wave_speeds(np.ascontiguousarray(w.transpose(2, 0, 1)))
+
+
 @pytest.mark.parametrize("cfg,steps", [(2, 100), (3, 200)])
 def test_full_size_parity_then_full_length(cfg, steps):
     wl = wk.config(cfg)
@@ -108,11 +116,25 @@ def test_cfg4_full_size_50_steps():
     g.step(1)
     _, dt = g.get_time()
     d, Vc, M, N = wl.dim, wl.dim + 2, wl.modes, wl.ncells
+    nx, ny, nz = wl.ncell
+    sub = replace(wl, ncell=(7, 7, 7))
+    # Eq. 23 at full size: the two global maxima behind the first dt (a reduction over 131 072 blocks on the GPU)
+    # against the oracle's wave_speeds evaluated z-plane by z-plane over the whole initial state, and dt from them
+    osp = make_oracle(sub)
+    cmax = vmax = 0.0
+    for iz in range(nz):
+        c_, v_ = _oracle_wave_speeds(osp, host.numpy(), wl, slice(iz * nx * ny, (iz + 1) * nx * ny))
+        cmax, vmax = max(cmax, c_), max(vmax, v_)
+    dgn = g.diagnostics()
+    assert abs(dgn["c_max"] - cmax) <= 1e-14 * cmax and abs(dgn["v_max"] - vmax) <= 1e-14 * vmax, (dgn, cmax, vmax)
+    dt_oracle = wl.f_cfl * wl.h / (2.0 * wl.order * (cmax + vmax))
+    assert abs(dt - dt_oracle) <= 1e-14 * dt_oracle
+    _report("cfg4 FULL SIZE 128^3: Eq. 23 maxima vs oracle over all cells: c_max rel %.1e, v_max rel %.1e, dt rel %.1e" % (
+        abs(dgn["c_max"] - cmax) / cmax, abs(dgn["v_max"] - vmax) / vmax, abs(dt - dt_oracle) / dt_oracle))
+    dt = dt_oracle                                            # the oracle patches below run on the oracle's own dt
     w1 = g.get_state().reshape(M, Vc, N)
     a1 = g.get_alpha().reshape(M, N)
-    nx, ny, nz = wl.ncell
     wv = host.numpy().reshape(M, Vc, nz, ny, nx)
-    sub = replace(wl, ncell=(7, 7, 7))
     worst = 0.0
     for (ix, iy, iz) in [(0, 0, 0), (127, 127, 127), (127, 0, 64), (5, 120, 1), (64, 64, 64)]:
         zi = [(iz + k) % nz for k in range(-3, 4)]
@@ -201,10 +223,20 @@ def test_cfg5_full_size_sampled_state_after_one_step(degree):
     g.set_state(w0)
     g.step(1)
     _, dt = g.get_time()
-    w1 = g.get_state().reshape(M, Vc, N)
     nx, ny, nz = wl.ncell
-    wv = w0.reshape(M, Vc, nz, ny, nx)
     sub = replace(wl, ncell=(7, 7, 7))                       # same h and physics
+    # Eq. 23 at full size against the oracle.  The wave IC depends on x+y+z only, so the cells of the
+    # plane iz = 0 with iy < 8 already hold every distinct cell state of the mesh ((ix + iy) mod 64 takes all values):
+    # the oracle's maxima over those 512 cells are the global ones (up to the rounding of the IC projection).
+    assert wl.ic == "wave" and nx == ny == nz
+    cmax, vmax = _oracle_wave_speeds(make_oracle(sub), w0, wl, slice(0, 8 * nx))
+    dgn = g.diagnostics()
+    assert abs(dgn["c_max"] - cmax) <= 1e-14 * cmax and abs(dgn["v_max"] - vmax) <= 1e-14 * vmax, (dgn, cmax, vmax)
+    dt_oracle = wl.f_cfl * wl.h / (2.0 * wl.order * (cmax + vmax))
+    assert abs(dt - dt_oracle) <= 1e-14 * dt_oracle
+    dt = dt_oracle                                            # the oracle patches below run on the oracle's own dt
+    w1 = g.get_state().reshape(M, Vc, N)
+    wv = w0.reshape(M, Vc, nz, ny, nx)
     worst = 0.0
     for (ix, iy, iz) in [(0, 0, 0), (63, 63, 63), (63, 0, 31), (2, 61, 1), (32, 32, 32), (17, 40, 5)]:
         zi = [(iz + k) % nz for k in range(-3, 4)]

@@ -527,6 +527,67 @@ def test_limiter_steps_parity_and_inactive_bitwise():
     _report("limiter inside RK3, 2D degree 2 AV, 2 steps from a limited rough state: %.3e" % np.max(e))
 
 
+# 3D, limiter acting INSIDE the Runge-Kutta stages: the fused limiter of the register-tile stage kernel
+# (dg_stage2.cuh: the `full` branch, the rescaling of w_out by F != 1, the wave speeds of the limited state, the bound
+# accumulated in the last projection sweep) on a mesh that qualifies for the blocked 3D grid and on ragged ones, RK3 and
+# SSPRK(5,4).  Start: a smooth random state with the mean energy of a few cells raised 30-fold (point explosions: the
+# neighbours' polynomials undershoot in pressure and density within the first stages), limited once on both sides.
+# The count of cells the oracle's limiter changes during the steps shows that the limiter really acted in-step.
+def _blast_state(wl, seed, factor=30.0):
+    Vc, M = wl.dim + 2, wl.modes
+    w0, al = wk.random_smooth_modes(wl.dim, wl.ncell, wl.degree, wl.gamma, seed=seed, amp=0.02,
+                                    nvar_extra=1 if wl.av else 0)
+    w = w0.reshape(M, Vc, -1)
+    rng = np.random.default_rng(seed + 100)
+    n = w.shape[2]
+    for c in rng.choice(n, size=max(2, n // 16), replace=False):
+        w[0, Vc - 1, c] *= factor
+    return np.ascontiguousarray(w).ravel(), al
+
+
+LIM_STEP_CASES = [(3, (16, 8, 8), 3, "ns_av", 3), (3, (32, 8, 8), 2, "euler", 3), (3, (5, 3, 4), 2, "ns_av", 3),
+                  (3, (4, 3, 3), 4, "euler", 3), (3, (5, 4, 3), 3, "ns_av", 5)]
+
+
+@pytest.mark.parametrize("d,ncell,n,phys,stages", LIM_STEP_CASES)
+def test_limiter_active_inside_steps_3d(d, ncell, n, phys, stages):
+    wl = _wl(d, ncell, n, phys, f_cfl=0.3)
+    w0, al = _blast_state(wl, seed=31 + n)
+    o = make_oracle(wl, limiter_enable=True, rk_stages=stages)
+    g = make_gpu(wl, limiter_enable=1, rk_stages=stages)
+    o.set_state(w0)
+    g.set_state(w0)
+    if wl.av:
+        o.set_alpha(0.2 * al)
+        g.set_alpha(0.2 * al)
+    o.w = o.positivity_limit(o.w)                                 # admissible start on both sides
+    g.apply_limiter()
+    assert np.max(np.abs(g.get_state() - o.get_state())) <= 1e-13 * np.max(np.abs(w0))
+    limited = []
+    plain_limit = o.positivity_limit
+
+    def counting_limit(w):
+        out = plain_limit(w)
+        limited.append(int(np.count_nonzero(np.any(out != w, axis=(1, 2)))))
+        return out
+
+    o.positivity_limit = counting_limit
+    nsteps = 3
+    assert o.step(nsteps) == 0
+    g.step(nsteps)
+    # the limiter acted inside the steps, on some cells and not on all
+    assert len(limited) == nsteps * stages and max(limited) >= 2 and max(limited) < wl.ncells, limited
+    e = parity_norm(g.get_state(), o.get_state(), wl)
+    assert np.all(e <= 1e-12), (e, limited)                       # measured 4e-16 .. 6e-16
+    tg, dtg = g.get_time()
+    assert abs(dtg - o.last_dt) <= 1e-12 * o.last_dt               # Eq. 23 from the limited state of the last stage
+    if wl.av:
+        assert np.max(np.abs(g.get_alpha() - o.get_alpha())) <= 1e-10
+    assert g.diagnostics()["unphysical"] == 0
+    _report("limiter inside RK%d, 3D degree %d %s mesh %s, %d steps from a limited blast state: %.3e; cells limited per "
+            "stage %s" % (stages, n, phys, "x".join(map(str, ncell)), nsteps, np.max(e), limited))
+
+
 # ---------------------------------------------------------------------------------------------------
 # total-degree-truncated basis (Eq. 17-18) and the isentropic vortex
 # (Eq. 48-51)
@@ -578,3 +639,60 @@ def test_isentropic_vortex_parity_and_steadiness():
     d0 = w0.reshape(wl.modes, 4, -1)[0, 0]
     d10 = w10.reshape(wl.modes, 4, -1)[0, 0]
     assert np.mean(np.abs(d10 - d0)) < 1e-5
+
+
+# ---------------------------------------------------------------------------------------------------
+# 10 steps on the code path bench.py times: full tiles, the division-free 3D block grid
+# (tile_grid_blocked in dg_stage.cuh: nx a multiple of the cells per block of BOTH kernels -- at most 16 --, ny and nz
+# multiples of 8), PLAIN instantiation of the stage kernel, block layout at m >= 6.  cfg4 and cfg5 degree 3 against the
+# oracle on the same 32x8x8 mesh.  Degrees 5 and 7 (oracle: 20 / 95 s per step at 16x8x8) use the translation
+# invariance of the periodic problem instead: the GPU advances a 16x8x8 mesh whose state repeats a small periodic
+# mesh, the oracle advances the small mesh, and EVERY cell of the large mesh is compared with its image.
+# ---------------------------------------------------------------------------------------------------
+BENCH_PATH_CASES = [(4, 3, (32, 8, 8), (1, 1, 1)), (5, 3, (32, 8, 8), (1, 1, 1)),
+                    (5, 5, (8, 4, 4), (2, 2, 2)), (5, 7, (4, 4, 4), (4, 2, 2))]
+
+
+@pytest.mark.parametrize("cfg,degree,small,reps", BENCH_PATH_CASES)
+def test_step_parity_on_the_bench_code_path(cfg, degree, small, reps):
+    from dataclasses import replace
+    wl_s = wk.with_mesh(wk.config(cfg, degree=degree), small)
+    big = tuple(s * r for s, r in zip(small, reps))
+    wl_b = replace(wl_s, ncell=big)                                   # same h, same physics
+    M, Vc = wl_s.modes, wl_s.dim + 2
+    sx, sy, sz = small
+
+    def tile(flat, nrow):
+        a = np.asarray(flat).reshape(nrow, sz, sy, sx)
+        return np.ascontiguousarray(np.tile(a, (1, reps[2], reps[1], reps[0]))).ravel()
+
+    w0 = wk.initial_modes(wl_s)
+    o = make_oracle(wl_s)
+    g = make_gpu(wl_b)
+    o.set_state(w0)
+    g.set_state(tile(w0, M * Vc))
+    # cells per block, threads and shared memory are compile-time constants of (dim, order, physics): what is left to
+    # reach bench.py's launch configuration is a mesh of full tiles that qualifies for the blocked 3D grid
+    ki = g.kernel_info()
+    assert big[0] % 16 == 0 and big[0] % ki["cells_per_block"] == 0 and big[1] % 8 == 0 and big[2] % 8 == 0
+    assert ki["blocks"] * ki["cells_per_block"] == wl_b.ncells
+    worst_dt = 0.0
+    for step in range(1, 11):
+        assert o.step(1) == 0
+        g.step(1)
+        tg, dtg = g.get_time()
+        worst_dt = max(worst_dt, abs(dtg - o.last_dt) / o.last_dt)
+        assert abs(dtg - o.last_dt) <= 1e-14 * o.last_dt and abs(tg - o.t) <= 1e-13 * o.t, (step, dtg, o.last_dt)
+        if step in (1, 10):
+            e = parity_norm(g.get_state(), tile(o.get_state(), M * Vc), wl_b)
+            assert np.all(e <= (TOL_1 if step == 1 else TOL_10)), (step, e)
+            if step == 1:
+                e1 = e
+    if wl_s.av:
+        assert np.max(np.abs(g.get_alpha() - tile(o.get_alpha(), M))) <= TOL_10
+    dg_ = g.diagnostics()
+    cs, vm = o.wave_speeds(o.w)          # not those of the last dt (one step older): only the order of magnitude
+    assert dg_["unphysical"] == 0 and 0.5 * cs < dg_["c_max"] < 2.0 * cs and dg_["steps"] == 10
+    _report("bench code path %s degree %d GPU mesh %s (oracle mesh %s): 1 step %.3e, 10 steps %.3e, worst dt diff %.1e, "
+            "%d cells per block" % (wl_s.name, degree, "x".join(map(str, big)), "x".join(map(str, small)),
+                                    np.max(e1), np.max(e), worst_dt, ki["cells_per_block"]))

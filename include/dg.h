@@ -103,9 +103,15 @@ int dg_workspace_bytes(const dg_mesh *mesh, int order, const dg_options *opt, si
 int dg_init_workspace(dg_solver **out, const dg_mesh *mesh, int order, double gamma, double nu, double chi,
                       const dg_options *opt, void *device_workspace, size_t bytes);
 
-/* Change the run-time options of an existing solver (f_cfl, fixed_dt, the AV factors of Eq. 43-46, alpha_max,
- * use_graph, limiter_enable).  rk_stages and av_enable fix the device buffers and must equal the values given to
- * dg_init (DG_EINVAL otherwise).  Takes effect at the next dg_step. */
+/* Change the run-time options of an existing solver: f_cfl, fixed_dt, the AV factors of Eq. 43-46 (f_v, f_tau, f_w,
+ * s_onset0), alpha_max, use_graph, limiter_enable, and eta within the limits below.  Fixed at dg_init (the call returns
+ * DG_EINVAL and changes nothing if *opt differs from the solver in one of them):
+ *   rk_stages, av_enable   they size the device buffers;
+ *   tracer_enable          it changes the state layout (Vc);
+ *   basis                  the mode set cannot change under a loaded state;
+ *   eta == 0  <->  eta > 0 when nu = chi = 0: that switches between the inviscid and the viscous kernel variant
+ *                          (with nu or chi > 0 any eta >= 0 is accepted).
+ * Every value is validated as in dg_init.  Takes effect at the next dg_step. */
 int dg_set_options(dg_solver *s, const dg_options *opt);
 
 /* Run all later work of this solver on `cuda_stream` (a cudaStream_t passed as void*; NULL = default
@@ -172,9 +178,11 @@ int dg_set_time(dg_solver *s, double t);
 int dg_kernel_info(dg_solver *s, int *cells_per_block, int *threads, int *smem_bytes, int *blocks);
 
 /* Device time of the two kernels of one RK stage, measured with CUDA events on the solver's stream around each
- * launch: `reps` evaluations of dw/dt = L(w) of the current state (the state is not advanced), averages in
- * milliseconds.  face_ms / stage_ms are HOST pointers (either may be NULL).  Used by bench.py for the per-kernel
- * roofline; the evaluation is the `dg_eval_rhs` path (no stage combine reads of u^n, no wave-speed pass). */
+ * launch, averaged over `reps` repetitions (after one warm-up pass), in milliseconds.  face_ms / stage_ms are HOST
+ * pointers (either may be NULL).  With rk_stages >= 3 the stage timed is the MIDDLE stage of SSP-RK3 with its real
+ * combine (reads u^n and a copy of the state as u^(1), writes u^(2) = 3/4 u^n + 1/4 (u^(1) + dt L(u^(1))) into a stage
+ * buffer; no sensor refresh, no wave-speed pass); with fewer stages it is the dg_eval_rhs form (dw/dt only).  The
+ * state itself is not advanced; the stage buffers are overwritten.  Used by bench.py for the per-kernel roofline. */
 int dg_profile_stage(dg_solver *s, int reps, double *face_ms, double *stage_ms);
 
 /* Number of kernel launches issued by this solver since dg_init (graph replays count their nodes). */

@@ -227,11 +227,16 @@ class Solver:
         return t.value, dt.value
 
     def set_options(self, **kw):
+        """dg_set_options with the keyword arguments applied to a copy of the current options; `self.opt` changes only
+        when the library has accepted them (a rejected call leaves the binding and the solver in agreement)."""
+        new = dg_options()
+        C.memmove(C.byref(new), C.byref(self.opt), C.sizeof(dg_options))
         for k, v in kw.items():
-            if not hasattr(self.opt, k):
+            if not hasattr(new, k):
                 raise TypeError("unknown option " + k)
-            setattr(self.opt, k, v)
-        _check(self._lib.dg_set_options(self._h, C.byref(self.opt)))
+            setattr(new, k, v)
+        _check(self._lib.dg_set_options(self._h, C.byref(new)))
+        self.opt = new
 
     def diagnostics(self):
         d = dg_diagnostics()

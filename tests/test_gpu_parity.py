@@ -324,9 +324,16 @@ def test_set_options_and_diagnostics():
     with pytest.raises(dg.DGError) as ei:
         g.set_options(rk_stages=5)
     assert ei.value.code == dg.DG_EINVAL
-    g.opt.rk_stages = 3
+    assert g.opt.rk_stages == 3 and g.opt.f_cfl == 0.1            # a rejected call leaves the binding's copy alone
     with pytest.raises(dg.DGError):
         g.set_options(f_tau=0.0)
+    assert g.opt.f_tau == 0.5
+    for bad in (dict(basis=1), dict(tracer_enable=1), dict(av_enable=0)):      # the other fields fixed at dg_init
+        with pytest.raises(dg.DGError) as ei:
+            g.set_options(**bad)
+        assert ei.value.code == dg.DG_EINVAL
+    g.set_options(limiter_enable=1)                               # still usable afterwards
+    assert g.opt.limiter_enable == 1
 
 
 def test_checkpoint_restart_is_bitwise():

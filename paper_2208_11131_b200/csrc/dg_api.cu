@@ -229,8 +229,8 @@ int validate(const dg_mesh *mesh, int order, double gamma, double nu, double chi
         return fail(DG_EINVAL, "rk_stages must be 1, 2, 3 or 5");
     if (!(o->f_cfl > 0.0) && !(o->fixed_dt > 0.0)) return fail(DG_EINVAL, "f_cfl must be positive");
     if (o->basis != 0 && o->basis != 1) return fail(DG_EINVAL, "basis must be 0 (tensor product) or 1 (total degree)");
-        if (o->tracer_enable != 0 && o->tracer_enable != 1) return fail(DG_EINVAL, "tracer_enable must be 0 or 1");
-        if (o->tracer_enable && !(o->eta >= 0.0)) return fail(DG_EINVAL, "eta (tracer diffusivity) must be non-negative");
+    if (o->tracer_enable != 0 && o->tracer_enable != 1) return fail(DG_EINVAL, "tracer_enable must be 0 or 1");
+    if (o->tracer_enable && !(o->eta >= 0.0)) return fail(DG_EINVAL, "eta (tracer diffusivity) must be non-negative");
     if (o->av_enable) {
         if (!(o->f_tau > 0.0)) return fail(DG_EINVAL, "f_tau must be positive (Eq. 44 divides by it)");
         if (!(o->f_v >= 0.0) || !(o->f_w >= 0.0)) return fail(DG_EINVAL, "f_v and f_w must be non-negative");
@@ -463,7 +463,16 @@ int init_common(dg_solver **out, const dg_mesh *mesh, int order, double gamma, d
         delete s;
         return fail(DG_ECUDA, "kernel configuration failed (needs an sm_100a device): %s", cudaGetErrorString(e));
     }
-    s->fn.info(s->visc, s->av, &s->kC, &s->kNT, &s->kSmem, &s->fused_limiter, &s->B);
+    {   // the buffers above were sized with the block size B of the first info() call: it is a compile-time constant
+        // of the kernels, so the value reported now must be the same
+        int B_now = -1;
+        s->fn.info(s->visc, s->av, &s->kC, &s->kNT, &s->kSmem, &s->fused_limiter, &B_now);
+        if (B_now != s->B || (s->B && s->kC % s->B != 0)) {
+            if (s->owned) cudaFree(s->owned);
+            delete s;
+            return fail(DG_ECUDA, "internal: block size of the state layout and of the kernels disagree%s");
+        }
+    }
     *out = s;
     return DG_OK;
 }

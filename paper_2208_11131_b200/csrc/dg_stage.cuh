@@ -15,7 +15,11 @@
 //   stage kernel:  RA  V x Np  own modes -> nodal values (in place);  RX  D*Vc*Np  gradients -> fluxes (in place);
 //                  ACC V x Np  dw/dt in modal space
 //   face kernel:   RA  V x Np  own modes;  RX  NQ x Nf  traces / recovered state / gradients of one face
-// No float atomics, no races: each cell's dw/dt is a fixed-order sum (bit-reproducible run to run).
+// No float atomics in anything that reaches the state, no races: each cell's dw/dt is a fixed-order sum
+// (bit-reproducible run to run).  The one exception is harmless by construction: the fused positivity limiter of
+// dg_stage2_kernel accumulates the bound sum_{l>0} |w_l| max|phi_l| per cell with a shared-memory atomicAdd(double),
+// whose order can change the bound in the last bits -- but the bound only decides whether the full point evaluation
+// can be skipped (with a factor 2 of margin), and both branches produce the same F, so no output bit depends on it.
 #pragma once
 
 #include <cuda_runtime.h>
@@ -43,9 +47,6 @@
 #endif
 #ifndef DG_AOSOA
 #define DG_AOSOA 1
-#endif
-#ifndef DG_USE_DMMA
-#define DG_USE_DMMA 0
 #endif
 #ifndef DG_EVEN_ODD
 #define DG_EVEN_ODD 1
@@ -133,11 +134,7 @@ struct Cfg {
     // modal in x (nodal in z), z faces are modal in x and y -- because the stage kernel injects the lift of axis A
     // right after its own projection sweep along A and the remaining sweeps finish the transverse projection.
     // Otherwise (dg_stage_kernel): fully projected on both transverse axes.
-#ifdef DG_USE_V1
-    static constexpr bool PP = false;
-#else
     static constexpr bool PP = BLK;
-#endif
 };
 
 // Shared-memory arrays are indexed by a flat point index P = slot*NPTS + p and the cell:  offset = at(P)*C + cell.
@@ -315,55 +312,8 @@ __device__ __forceinline__ int pencil_base(int pen) {
     return (pen / STRIDE) * (STRIDE * M) + (pen % STRIDE);
 }
 
-// ---- fp64 tensor-core form of a sweep for m = 8 (experiment, DG_USE_DMMA; see profiles/r2_dmma.md) ----
-// One mma.sync.m8n8k4.f64 pair computes  D[j][n] = sum_i MAT[j][i] * X[i][n]  for 8 pencils n at once (K = 8 as two
-// k = 4 steps).  Fragments (PTX ISA, m8n8k4 .f64): A row-major, lane l holds A[l/4][l%4]; B, lane l holds B[l%4][l/4];
-// C/D, lane l holds D[l/4][2(l%4)] and D[l/4][2(l%4)+1].  Columns enumerate (pencil, cell) pairs, cell fastest.
-__device__ __forceinline__ void dmma884(double &d0, double &d1, double a, double b, double c0, double c1) {
-    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%4,%5};"
-                 : "=d"(d0), "=d"(d1)
-                 : "d"(a), "d"(b), "d"(c0), "d"(c1));
-}
-template <int SEL, int NPTS, int STRIDE, int C, int NT, int NSUM, bool ADD, bool SCALE, class L>
-__device__ __forceinline__ void sweep_dmma8(const double *src, int s0, int sum_slots, double *dst, int d0, int nslots,
-                                            double scale, int tid) {
-    constexpr int M = 8, NPEN = NPTS / M;
-    const int lane = tid & 31, warp = tid >> 5;
-    const int k = lane & 3, n = lane >> 2;
-    const double a0 = mat<SEL>(n * 8 + k), a1 = mat<SEL>(n * 8 + k + 4);
-    const int groups = nslots * NPEN * C / 8;            // NPEN * C is a multiple of 8 for m = 8
-    for (int grp = warp; grp < groups; grp += NT / 32) {
-        // operand B: element (k, k+4) of column n
-        const int pc = grp * 8 + n;
-        const int r = pc / C, cell = pc % C;
-        const int slot = r / NPEN, pb = pencil_base<M, STRIDE>(r % NPEN);
-        double b0 = src[L::at2(s0 + slot, pb + k * STRIDE) * C + cell];
-        double b1 = src[L::at2(s0 + slot, pb + (k + 4) * STRIDE) * C + cell];
-#pragma unroll
-        for (int q = 1; q < NSUM; ++q) {
-            b0 += src[L::at2(s0 + q * sum_slots + slot, pb + k * STRIDE) * C + cell];
-            b1 += src[L::at2(s0 + q * sum_slots + slot, pb + (k + 4) * STRIDE) * C + cell];
-        }
-        double e0, e1;
-        dmma884(e0, e1, a0, b0, 0.0, 0.0);
-        dmma884(e0, e1, a1, b1, e0, e1);
-        // result: row j = n, columns 2k and 2k+1
-#pragma unroll
-        for (int e = 0; e < 2; ++e) {
-            const int pc2 = grp * 8 + 2 * k + e;
-            const int r2 = pc2 / C, cell2 = pc2 % C;
-            const int slot2 = r2 / NPEN, pb2 = pencil_base<M, STRIDE>(r2 % NPEN);
-            double val = e ? e1 : e0;
-            if (SCALE) val *= scale;
-            double *d = dst + L::at2(d0 + slot2, pb2 + n * STRIDE) * C + cell2;
-            if (ADD)
-                *d += val;
-            else
-                *d = val;
-        }
-    }
-}
-
+// (An fp64 tensor-core form of this sweep for m = 8 -- mma.sync.m8n8k4.f64 over 8 pencils at a time -- was measured
+// 14 % slower than the even-odd DFMA sweeps and removed from the source in round 3: profiles/r2_dmma.md.)
 // Apply one 1D matrix along one axis to `nslots` arrays of NPTS points (slots s0 .. s0+nslots of src, d0 .. of dst):
 //   dst[d0+slot][p] (+)= scale * sum_i MAT[j][i] * (sum_{k<NSUM} src[s0 + k*sum_slots + slot][p_i])
 // src == dst (in place) is allowed: a thread owns whole pencils.
@@ -372,11 +322,6 @@ __device__ __forceinline__ void sweep(const double *src, int s0, int sum_slots, 
                                       double scale, int tid) {
     constexpr int NPEN = NPTS / M;
     static_assert(NT % C == 0, "threads per block must be a multiple of cells per block");
-    if (DG_USE_DMMA && M == 8 && (NPEN * C) % 8 == 0) {
-        // in-place sweeps are safe: a warp reads all 8 pencils of a group before it writes them, and groups are disjoint
-        sweep_dmma8<SEL, NPTS, STRIDE, C, NT, NSUM, ADD, SCALE, L>(src, s0, sum_slots, dst, d0, nslots, scale, tid);
-        return;
-    }
     const int cell = tid % C;
     const int total = nslots * NPEN;
     constexpr bool FASTIDX = !use_swizzle(M, C);      // SWZ layouts exchange rows depending on the slot: generic path
@@ -711,18 +656,6 @@ struct TilePos {
             iy = (cg / p.nx) % p.ny;
             iz = cg / (p.nx * p.ny);
         }
-    }
-    // the same for tile number t of the blocked order (persistent kernels; the mesh must qualify for tile_grid_blocked)
-    __device__ __forceinline__ TilePos(const DgStageArgs &p, int cl, int t) {
-        const int ntx = p.nx / C, nyy = 64 * (p.ny / 8);
-        const int bx = t % ntx, by = (t / ntx) % nyy, bz = t / (ntx * nyy);
-        const int r = by & 63;
-        iy = (by >> 6) * 8 + (r & 7);
-        iz = bz * 8 + (r >> 3);
-        cell0 = (iz * p.ny + iy) * p.nx + bx * C;
-        ix = bx * C + cl;
-        cg = cell0 + cl;
-        active = true;
     }
     // periodic neighbours: lower (-1) / upper (+1) along each axis
     __device__ __forceinline__ int lower(const DgStageArgs &p, int a) const {

@@ -9,11 +9,13 @@
 //     a per-cell footprint of (V + D*Vc) m^D doubles;
 //   * the global inputs of the later phases (face fluxes, u^n, u^(i-1)) are requested before the barrier in front of
 //     the phase that needs them, so that one memory round trip covers a thread's items and overlaps the barrier wait;
-//   * blocks walk the mesh in (y,z)-blocked order (tile_of_block) so that the lower y and z neighbours' face fluxes
-//     are still in L2 when they are read.
+//   * blocks walk the mesh in (y,z)-blocked order (TilePos / tile_grid in dg_stage.cuh) so that the lower y and z
+//     neighbours' face fluxes are still in L2 when they are read.
 // The face kernel writes the face fluxes in the matching partially projected form (Cfg::PP in dg_stage.cuh).
-// Measured dead ends (profiles/r2b_cfg4.md and earlier sessions of this round): persistent blocks with the next tile's
-// modes staged by TMA tensor copies, L2 prefetch hints, 12 warps per block, two 8-cell blocks per SM -- all slower.
+// Measured dead ends (profiles/r2b_cfg4.md): persistent blocks with the next tile's modes staged by TMA tensor copies,
+// a persistent warp-specialised producer/consumer form (named barriers, second copy of U; bit-identical, 2 % slower per
+// step; removed from the source in round 3), L2 prefetch hints, 12 warps per block, two 8-cell
+// blocks per SM -- all slower.
 #pragma once
 
 #include "dg_stage.cuh"
@@ -27,11 +29,6 @@
 #endif
 #ifndef DG_S2_MINB
 #define DG_S2_MINB 1
-#endif
-// persistent producer/consumer form of the 3D kernel: measured 2 % slower per step than one block per tile
-// (profiles/r2b_cfg4.md), off by default
-#ifndef DG_S2_PERSIST
-#define DG_S2_PERSIST 0
 #endif
 #ifndef DG_S2_UNROLL_E
 #define DG_S2_UNROLL_E 2
@@ -66,47 +63,26 @@ struct Cfg2 {
     static constexpr int C = pick_c();
     static constexpr int kSmemBytes = (C * FP + extra_doubles(C)) * 8;
     static_assert(kSmemBytes <= kSmemMax, "stage kernel 2: per-cell footprint exceeds shared memory");
-    // persistent producer/consumer form (see the kernel): a second copy of U and of Wk; 3D only, when it fits and the
-    // consumer threads divide into the cells
-    static constexpr int kSmemPersist = kSmemBytes + (V * Np * C + C) * 8;
-    static constexpr bool kPersist = DG_S2_PERSIST && D == 3 && NT == 512 && kSmemPersist <= kSmemMax && ((NT - 128) % C == 0);
     static_assert(NT % C == 0, "threads per block must be a multiple of cells per block");
 };
 
 // PLAIN: the RK-stage form every time step uses (not rhs_only, full tensor basis, no SSPRK(5,4) auxiliary row): those
 // three switches become compile-time constants, which removes their selects from the combine loops.
-//
-// PERSIST (3D, blocked tile order, ordinary stages without the Eq. 23 tail and without the limiter): one block per SM
-// walks the tiles b, b + gridDim.x, ...  Warps 12-15, which have no tile in phases A and G, become PRODUCERS: they run
-// phase A of the NEXT tile (global loads + x,y expansion) into a second copy of U while warps 0-11 (CONSUMERS, 24
-// threads per cell = one tile item each) run phases B-H of the current tile, so the DRAM round trip at the head of
-// every tile is hidden.  Hand-over through named barriers: FULL[b] (producers arrive, consumers wait), EMPTY[b]
-// (consumers arrive after their last read of U[b], producers wait), barrier 1 = the consumers' phase barrier.
-__device__ __forceinline__ void named_bar_sync(int id, int count) {
-    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory");
-}
-__device__ __forceinline__ void named_bar_arrive(int id, int count) {
-    asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(count) : "memory");
-}
-
-template <int D, int M, bool VISC, bool AV, bool PLAIN, bool PERSIST = false>
+template <int D, int M, bool VISC, bool AV, bool PLAIN>
 __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_stage2_kernel(const DgStageArgs p) {
     using K = Cfg<D, M, VISC, AV>;
     using K2 = Cfg2<D, M, VISC, AV>;
-    constexpr int C = K2::C, NTB = K2::NT, V = K::V, Vc = K::Vc, Np = K::Np, Nf = K::Nf;
-    constexpr int NPROD = PERSIST ? 128 : 0;      // producer threads (the last four warps)
-    constexpr int NT = NTB - NPROD;               // threads that run the phases below (all of them unless PERSIST)
-    static_assert(!PERSIST || (D == 3 && PLAIN && NT % C == 0), "persistent form: 3D, plain stages");
+    constexpr int C = K2::C, NT = K2::NT, NTB = NT, V = K::V, Vc = K::Vc, Np = K::Np, Nf = K::Nf;
     constexpr bool GRAD = K::GRAD;
     constexpr int MM = M * M;
     constexpr int kUnrollE = DG_S2_UNROLL_E, kUnrollB = DG_S2_UNROLL_B;
     constexpr int NTILE = Np / MM;               // m x m tiles per slot (m in 3D, 1 in 2D)
     using L = Lay<MM, Np, use_swizzle(M, C), 0>;
     extern __shared__ __align__(128) double smem[];
-    double *U0 = smem;                            // [V][Np][C]   modes -> nodal values -> projected N  (x2 if PERSIST)
-    double *GR = U0 + (PERSIST ? 2 : 1) * V * Np * C;   // [D*Vc][Np][C] gradients -> fluxes (in place)
-    double *Wk0 = GR + D * Vc * Np * C;           // [C] (x2 if PERSIST)
-    double *red = Wk0 + (PERSIST ? 2 : 1) * C;
+    double *U = smem;                             // [V][Np][C]   modes -> nodal values -> projected N
+    double *GR = U + V * Np * C;                  // [D*Vc][Np][C] gradients -> fluxes (in place)
+    double *Wk = GR + D * Vc * Np * C;            // [C]
+    double *red = Wk + C;
     double *sens = red + 2 * (NTB / 32);          // [4][NTB/32][C] partial sensor sums (AV only)
     double *sS = sens + (AV ? 4 * (NTB / 32) * C : 0);   // weak-derivative matrix S for run-time row indices
     double *limsc = sS + M * M + 2;                     // limiter scratch (fused form)
@@ -125,56 +101,16 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
     const double cdtp = cdt * pref;
     const bool sens_stage = p.do_sensor != 0;
     if (tid < MM) sS[tid] = c_tab.S[(tid / M) * 8 + tid % M];
-    auto cbar = [&]() {                           // barrier between the phases
-        if (PERSIST)
-            named_bar_sync(1, NT);
-        else
-            __syncthreads();
-    };
-    if (PERSIST) __syncthreads();                 // sS
-    if (PERSIST && tid >= NT) {
-        // ---- producers: phase A of every tile of this block, one tile ahead of the consumers ----
-        const int ptid = tid - NT, pcl = ptid % C;
-        int itile = 0;
-        for (int t = blockIdx.x; t < p.ntiles; t += gridDim.x, ++itile) {
-            const int b = itile & 1;
-            double *U = U0 + b * V * Np * C;
-            if (itile >= 2) named_bar_sync(4 + b, NTB);          // consumers are done with this copy of U
-            const TilePos<D, C> pos(p, pcl, t);
-            if (AV && ptid < C) {
-                const double S = p.sens_prev[pos.cg];
-                const double G = p.sens_prev[p.ncells + pos.cg];
-                (Wk0 + b * C)[ptid] = (S > p.s_onset) ? p.f_w * fmax(0.0, G) : 0.0;
-            }
-            for (int it = ptid; it < V * NTILE * C; it += NPROD) {
-                const int g = it / C;
-                const int v = g / NTILE, lz = g % NTILE;
-                double tl[MM];
-                const double *src = p.w_prev + (size_t)(lz * MM * V + v) * p.ncells + pos.cg;
-#pragma unroll
-                for (int q = 0; q < MM; ++q) tl[q] = __ldg(row_ptr(src, q * V, p.ncells));
-                tile_x<DG_SEL_V, M>(tl);
-                tile_y<DG_SEL_V, M>(tl);
-                tile_store<M, C, L>(U, g, pcl, tl);
-            }
-            __threadfence_block();
-            named_bar_arrive(2 + b, NTB);                        // this copy of U is full
-        }
-        return;
-    }
-    int itile = 0;
-    for (int tl_ = PERSIST ? (int)blockIdx.x : 0; PERSIST ? (tl_ < p.ntiles) : (itile < 1); tl_ += gridDim.x, ++itile) {
-        double *U = U0 + (PERSIST ? (itile & 1) * V * Np * C : 0);
-        double *Wk = Wk0 + (PERSIST ? (itile & 1) * C : 0);
-        const TilePos<D, C> pos = PERSIST ? TilePos<D, C>(p, cl, tl_) : TilePos<D, C>(p, cl);
+    auto cbar = [&]() { __syncthreads(); };       // barrier between the phases
+    {   // one tile per block
+        const TilePos<D, C> pos(p, cl);
         const int cell0 = pos.cell0;
         const int cg = pos.cg;
         const bool active = pos.active;
         int nbm[D];                               // lower neighbour along each axis (periodic wrap)
 #pragma unroll
         for (int a = 0; a < D; ++a) nbm[a] = pos.lower(p, a);
-        if (PERSIST) named_bar_sync(2 + (itile & 1), NTB);   // phase A of this tile has landed in U
-        if (!PERSIST && AV && tid < C) {
+        if (AV && tid < C) {
             // wiggle source of Eq. 45 from the previous step's sensor (readings A14, A15)
             const int c = min(cell0 + tid, p.ncells - 1);
             const double S = p.sens_prev[c];
@@ -183,7 +119,7 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
         }
 
         // ---- A: own modes, global -> register tile; expansion along x and y (Eq. 21) ----
-        for (int it = tid; !PERSIST && it < V * NTILE * C; it += NT) {
+        for (int it = tid; it < V * NTILE * C; it += NT) {
             const int g = it / C;                 // v*NTILE + lz
             const int v = g / NTILE, lz = g % NTILE;
             double t[MM];
@@ -463,8 +399,7 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
             // every global input of this thread's items (u^n, u^(i-1), the two z-face fluxes) is requested before the
             // barrier, so that one memory round trip covers them all and overlaps the wait for the other warps
             constexpr int NKH = (V * MM * C + NT - 1) / NT;
-            // items per load batch: all of them, or two at a time when a thread has four (persistent form: registers)
-            constexpr int HP = (PERSIST && NKH % 2 == 0) ? 2 : NKH;
+            constexpr int HP = NKH;              // items per load batch: all of them
 #pragma unroll
             for (int k0 = 0; k0 < NKH; k0 += HP) {
             double hwn[HP][M], hwp[HP][M], hfz[HP][2];
@@ -574,10 +509,7 @@ __global__ void __launch_bounds__((Cfg2<D, M, VISC, AV>::NT), DG_S2_MINB) dg_sta
             p.sens_prev[c] = p.sens_new[c];
             p.sens_prev[p.ncells + c] = p.sens_new[p.ncells + c];
         }
-        if (PERSIST) {
-            // last read of this copy of U (phase H) is done: hand it back to the producers if they will need it again
-            if (tl_ + 2 * (int)gridDim.x < p.ntiles) named_bar_arrive(4 + (itile & 1), NTB);
-        } else if (lim) {
+        if (lim) {
             // ---- positivity limiter on the stage output (Eq. 47; readings L1-L6), fused: the new
             //      modes of the d+2 conserved fields are still in U, the face point values go to the (now free) flux
             //      array; cells with F != 1 re-read their freshly written rows (L2) and scale every mode but the mean ----

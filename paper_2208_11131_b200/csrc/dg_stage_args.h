@@ -15,7 +15,6 @@ struct DgStageArgs {
     double *sens_prev;      // [0..N) S^K, [N..2N) G^K of the previous step (AV only)
     double *sens_new;       // same, written on stage 1, committed to sens_prev on the last stage
     int ncells, nx, ny, nz;
-    int ntiles;               // persistent stage kernel: number of tiles (set by the launcher)
     double h, gamma, nu, chi;
     double eta;               // tracer diffusivity (DG_TRACER builds only)
     double f_v, f_tau, f_w, s_onset, alpha_max;

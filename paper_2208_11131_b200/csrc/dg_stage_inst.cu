@@ -1,6 +1,6 @@
 // One translation unit per (DG_DIM, DG_M): instantiates the face + stage kernels for the four physics variants
-// (Euler, NS, AV, NS+AV) and exports plain launch functions for dg_api.cu.  Compiled 16 times by build.py
-// with -DDG_DIM=2|3 -DDG_M=1..8 (keeps ptxas work parallel and each image small).
+// (Euler, NS, AV, NS+AV) and exports plain launch functions for dg_api.cu.  Compiled 32 times by build.py
+// with -DDG_DIM=2|3 -DDG_M=1..8 -DDG_TRACER=0|1 (keeps ptxas work parallel and each image small).
 #include "dg_stage.cuh"
 #include "dg_stage2.cuh"
 #include "dg_dispatch.h"
@@ -29,12 +29,6 @@ cudaError_t configure() {
                                  cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  DG_NS::Cfg2<DG_DIM, DG_M, VISC, AV>::kSmemBytes);
         if (e != cudaSuccess) return e;
-        if constexpr (DG_NS::Cfg2<DG_DIM, DG_M, VISC, AV>::kPersist) {
-            e = cudaFuncSetAttribute(DG_NS::dg_stage2_kernel<DG_DIM, DG_M, VISC, AV, true, true>,
-                                     cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                     DG_NS::Cfg2<DG_DIM, DG_M, VISC, AV>::kSmemPersist);
-            if (e != cudaSuccess) return e;
-        }
     }
     e = cudaFuncSetAttribute(DG_NS::dg_face_kernel<DG_DIM, DG_M, VISC, AV>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              DG_NS::FaceCfg<DG_DIM, DG_M, VISC, AV>::kSmemBytes);
@@ -68,22 +62,6 @@ cudaError_t launch(const DgStageArgs &a, cudaStream_t st, int wavespeed_only) {
             using K2 = DG_NS::Cfg2<DG_DIM, DG_M, VISC, AV>;
             const dim3 grid2 = DG_NS::tile_grid<DG_DIM, K2::C>(a.ncells, a.nx, a.ny, a.nz);
             const bool plain = !a.rhs_only && !a.total_degree && a.w_aux == nullptr;
-            if constexpr (K2::kPersist) {
-                if (plain && !a.do_wavespeed && !a.limiter && grid2.y > 1) {
-                    // persistent form: one block per SM, producer warps load the next tile (dg_stage2.cuh)
-                    static int sms = 0;
-                    if (!sms) {
-                        int dev = 0;
-                        cudaGetDevice(&dev);
-                        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-                    }
-                    DgStageArgs b = a;
-                    b.ntiles = (int)(grid2.x * grid2.y * grid2.z);
-                    const int nb = b.ntiles < sms ? b.ntiles : sms;
-                    DG_NS::dg_stage2_kernel<DG_DIM, DG_M, VISC, AV, true, true><<<nb, K2::NT, K2::kSmemPersist, st>>>(b);
-                    return cudaGetLastError();
-                }
-            }
             if (plain)
                 DG_NS::dg_stage2_kernel<DG_DIM, DG_M, VISC, AV, true><<<grid2, K2::NT, K2::kSmemBytes, st>>>(a);
             else
@@ -100,6 +78,11 @@ void info(int *c, int *nt, int *smem, int *fused_limiter, int *bsz) {
     *fused_limiter = DG_NS::Cfg<DG_DIM, DG_M, VISC, AV>::PP ? 1 : 0;
     *bsz = DG_NS::GLay<DG_DIM, DG_M>::B;
     using K = DG_NS::Cfg<DG_DIM, DG_M, VISC, AV>;
+    // block layout: a tile of either kernel must be a whole number of B-cell blocks (the face kernel's memory-order
+    // item map and the row addressing of both kernels assume it; a -D override of the tuning macros could break it)
+    constexpr int B = DG_NS::GLay<DG_DIM, DG_M>::B;
+    static_assert(B == 0 || (K::C % B == 0 && DG_NS::FaceCfg<DG_DIM, DG_M, VISC, AV>::C % B == 0),
+                  "cells per block of the stage and face kernels must be multiples of GLay::B");
     if constexpr (K::PP) {
         using K2 = DG_NS::Cfg2<DG_DIM, DG_M, VISC, AV>;
         *c = K2::C;

@@ -172,6 +172,63 @@ def aggregate(local_units: float, local_seconds: float, world: int, dist=None, d
     return float(u.item()) / float(t.item()), float(t.item())
 
 
+def time_entry(name, wl, label, limiter, host_state, steps, warmup, dev, stream, local, hbm_gbs):
+    """One line of the `sweep`: W warm-up + K timed RK3 steps of `wl` (CUDA events on the launch stream, own clock
+    samples), per-kernel times, both roofline fractions.  Same method as the headline run."""
+    import torch
+    from paper_2208_11131_b200 import dg
+    solver = dg.from_workload(wl, **({"limiter_enable": 1} if limiter else {}))
+    solver.set_state(host_state)
+    solver.step(warmup)
+    torch.cuda.synchronize(dev)
+    sampler = ClockSampler(index=local)
+    sampler.start()
+    n0 = solver.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    solver.step_async(steps)
+    e1.record(stream)
+    e1.synchronize()
+    torch.cuda.synchronize(dev)
+    clocks = sampler.stop()
+    solver.sync()
+    launches = solver.launch_count() - n0
+    t_dev = e0.elapsed_time(e1) * 1e-3
+    t_stage = t_dev / (3 * steps)
+    face_ms, stage_ms = solver.profile_stage(3)
+    info = solver.kernel_info()
+    solver.free()
+    visc = wl.nu > 0 or wl.chi > 0
+    r = rl.roofline(wl.dim, wl.m, visc, wl.av, wl.ncells, t_stage, hbm_gbs, rl.NOMINAL_FP64_TFLOPS, count="survey")
+    rr = rl.roofline(wl.dim, wl.m, visc, wl.av, wl.ncells, t_stage, hbm_gbs, rl.NOMINAL_FP64_TFLOPS)
+    key = "alu_frac" if r["bound"] == "alu" else "hbm_frac"
+    return {"name": name, "workload": label + (" + positivity limiter" if limiter else ""),
+            "value": float(wl.ncells) * wl.modes * wl.nvar * 3 * steps / t_dev, "unit": UNIT,
+            "steps": steps, "warmup": warmup, "ms_per_step": t_dev / steps * 1e3, "ms_per_stage": t_stage * 1e3,
+            "bound": r["bound"], "frac": r[key], "frac_refined": rr[key], "alu_frac": r["alu_frac"],
+            "hbm_frac": r["hbm_frac"], "t_fp64_ms": r["t_alu_ms"], "t_hbm_ms": r["t_hbm_ms"],
+            "alg_flops_per_cell": r["flops_per_launch"] / wl.ncells, "alg_bytes_per_cell": r["bytes_per_launch"] / wl.ncells,
+            "kernels": {"face_ms": face_ms, "stage_ms": stage_ms}, "gpu_launches": int(launches), "launch": info,
+            "clocks": clocks}
+
+
+def run_sweep(args, dev, stream, local, cfg4_host_state, hbm_gbs):
+    """The other lines the >= 60 % target of north_star is judged on, driver-timed with the
+    headline: the paper's timing workload (cfg4 + positivity limiter) and the second 3D config, cfg5,
+    at degrees 3, 5 and 7.  Each entry: 3 warm-up + 10 timed steps."""
+    import torch
+    out = []
+    wl4, label4 = pick_workload("cfg4", None)
+    out.append(time_entry("cfg4_limiter", wl4, label4, True, cfg4_host_state, 10, 3, dev, stream, local, hbm_gbs))
+    for degree in (3, 5, 7):
+        wl, label = pick_workload("cfg5", degree)
+        host = torch.empty(wl.nvar_conserved * wl.modes * wl.ncells, dtype=torch.float64, pin_memory=True)
+        wk.initial_modes_wave_by_shift(wl, out=host.numpy())
+        out.append(time_entry("cfg5_n%d" % degree, wl, label, False, host, 10, 3, dev, stream, local, hbm_gbs))
+        del host
+    return out
+
+
 def run_gpu(args):
     import torch
     import torch.distributed as dist
@@ -250,7 +307,10 @@ def run_gpu(args):
     face_ms, stage_ms = solver.profile_stage(3)              # per-kernel device time, events around each launch
     fp64_meas = dg.measure_fp64_peak(4096, stream.cuda_stream) / 1e12
     visc = wl.nu > 0 or wl.chi > 0
-    r = rl.roofline(wl.dim, wl.m, visc, wl.av, wl.ncells, t_stage, hbm_gbs, rl.NOMINAL_FP64_TFLOPS)
+    # frac follows SURVEY.md 8(d) AS WRITTEN; frac_refined uses this builder's count (transverse face sweeps added,
+    # point-wise constants counted from the source: DESIGN.md section 6)
+    r = rl.roofline(wl.dim, wl.m, visc, wl.av, wl.ncells, t_stage, hbm_gbs, rl.NOMINAL_FP64_TFLOPS, count="survey")
+    rr = rl.roofline(wl.dim, wl.m, visc, wl.av, wl.ncells, t_stage, hbm_gbs, rl.NOMINAL_FP64_TFLOPS)
     fl_face = rl.face_kernel_flops_per_cell(wl.dim, wl.m, visc, wl.av) * wl.ncells
     fl_stage = rl.stage_kernel_flops_per_cell(wl.dim, wl.m, visc, wl.av) * wl.ncells
     by_face, by_stage = (b * wl.ncells for b in rl.kernel_bytes_per_cell(wl.dim, wl.m, wl.av))
@@ -263,6 +323,9 @@ def run_gpu(args):
                 "peak_source": "%s HBM copy (MEASURED_PEAKS.json)" % which}
     tr = TRAFFIC_BYTES.get((args.workload, wl.degree))
     roof.update({
+        "frac_refined": rr["alu_frac"] if r["bound"] == "alu" else rr["hbm_frac"],
+        "alg_flops_per_cell_refined": rr["flops_per_launch"] / wl.ncells,
+        "count": "frac: SURVEY.md 8(d) formula as written; frac_refined: builder's count (roofline.py)",
         "traffic": (tr["face"] + tr["stage"]) if tr else None,
         "traffic_source": (tr["source"] + " (committed capture, not live)") if tr else None,
         "scope": "whole RK stage = dg_face_kernel + dg_stage kernel, timed region / (3 * steps)",
@@ -282,6 +345,12 @@ def run_gpu(args):
                     "implementation bytes = what the two-kernel design must move (state read twice, flux buffer), "
                     "not the algorithmic bytes of the headline"},
         "fp64_peak_measured_tflops": fp64_meas, "hbm_peak_gbs": hbm_gbs})
+    sweep = None
+    if world == 1 and args.workload == "cfg4" and args.degree is None and not args.limiter and not args.no_sweep:
+        solver.free()
+        del solver
+        torch.cuda.empty_cache()
+        sweep = run_sweep(args, dev, stream, local, host_in, hbm_gbs)
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         nproc = max(1, min(os.cpu_count() or 1, 64))
@@ -304,7 +373,7 @@ def run_gpu(args):
         "field_dof_per_s": value / wl.nvar,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": nstate * 8, "d2h_bytes_per_step": nstate * 8,
                 "steps": e2e_steps, "api": "dg_set_state(host) + dg_step(1) + dg_get_state(host), pinned buffers"},
-        "gpu_launches": int(launches), "clocks": clocks, "roofline": roof, "cpu_baseline": cpu,
+        "gpu_launches": int(launches), "clocks": clocks, "roofline": roof, "sweep": sweep, "cpu_baseline": cpu,
         "conserved_totals": [float(x) for x in totals],
     }
     print(json.dumps(line))
@@ -363,6 +432,8 @@ def main():
     ap.add_argument("--degree", type=int, default=None)
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-sweep", action="store_true",
+                    help="skip the `sweep` entries (cfg4 + limiter, cfg5 at degrees 3, 5, 7) of the default cfg4 run")
     ap.add_argument("--limiter", action="store_true",
                     help="positivity limiter on (with cfg4: the paper's timing workload NS + AV + limiter, PAPER.md:800)")
     args = ap.parse_args()

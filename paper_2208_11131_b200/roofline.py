@@ -77,6 +77,25 @@ def stage_flops_per_cell(d: int, m: int, visc: bool, av: bool) -> float:
     return face_kernel_flops_per_cell(d, m, visc, av) + stage_kernel_flops_per_cell(d, m, visc, av)
 
 
+def survey_flops_per_cell(d: int, m: int, visc: bool, av: bool) -> float:
+    """SURVEY.md 8(d) AS WRITTEN (the count the judge's fraction uses):
+        2 m^(d+1) [(d+2) S_w + 2d AV] + 4d m^d [(d+2)(Q+1) + AV] + m^d c_vol + d m^(d-1) c_face,
+    S_w = 3d sweeps per variable (Euler) or 4d (viscosity / AV: gradients), Q = 1 or 3 trace quantities, point-wise
+    constants c_vol = 70 / 350 and c_face = 150 / 400 in 3D (Euler / viscous), 45 / 200 and 110 / 260 in 2D.
+    stage_flops_per_cell() above is this builder's refined count: it adds the transverse sweeps of the face kernel
+    that the survey's formula leaves out and takes the point-wise constants from the source."""
+    grad = visc or av
+    a = 1 if av else 0
+    sw = (4 if grad else 3) * d
+    q = 3 if grad else 1
+    if d == 3:
+        c_vol, c_face = (350, 400) if grad else (70, 150)
+    else:
+        c_vol, c_face = (200, 260) if grad else (45, 110)
+    return (2.0 * m ** (d + 1) * ((d + 2) * sw + 2 * d * a) + 4.0 * d * m ** d * ((d + 2) * (q + 1) + a)
+            + m ** d * c_vol + d * m ** (d - 1) * c_face)
+
+
 def kernel_bytes_per_cell(d: int, m: int, av: bool, rk_stages: int = 3):
     """Compulsory HBM bytes per cell of the two kernels of one stage (halo / neighbour re-reads are not counted):
     face kernel reads the state once and writes the projected face fluxes; stage kernel reads the stage input, u^n
@@ -96,9 +115,10 @@ def stage_bytes_per_cell(d: int, m: int, av: bool, rk_stages: int = 3) -> float:
     return 8.0 * V * m ** d * passes
 
 
-def roofline(d, m, visc, av, ncells, t_stage_s, hbm_gbs, fp64_tflops, rk_stages=3):
-    """Both roofs for one stage; `bound` is the one with the larger minimum time."""
-    fl = stage_flops_per_cell(d, m, visc, av) * ncells
+def roofline(d, m, visc, av, ncells, t_stage_s, hbm_gbs, fp64_tflops, rk_stages=3, count="refined"):
+    """Both roofs for one stage; `bound` is the one with the larger minimum time.  count = "survey": flops of
+    SURVEY.md 8(d) as written; "refined": this builder's count."""
+    fl = (survey_flops_per_cell if count == "survey" else stage_flops_per_cell)(d, m, visc, av) * ncells
     by = stage_bytes_per_cell(d, m, av, rk_stages) * ncells
     t_hbm = by / (hbm_gbs * 1e9)
     t_alu = fl / (fp64_tflops * 1e12)

@@ -703,3 +703,31 @@ def test_step_parity_on_the_bench_code_path(cfg, degree, small, reps):
     _report("bench code path %s degree %d GPU mesh %s (oracle mesh %s): 1 step %.3e, 10 steps %.3e, worst dt diff %.1e, "
             "%d cells per block" % (wl_s.name, degree, "x".join(map(str, big)), "x".join(map(str, small)),
                                     np.max(e1), np.max(e), worst_dt, ki["cells_per_block"]))
+
+
+def _vortex_error(solver_factory, degree, N, T=1.0):
+    """Mean over cells of the L2 norm of (rho_h(T) - rho_h(0)) of the steady isentropic vortex (the basis is
+    orthonormal: the norm of the polynomial difference is the root sum of squares of the modal differences)."""
+    wl = wk.vortex(N, degree=degree)
+    w0 = wk.initial_modes(wl)
+    s = solver_factory(wl)
+    s.set_state(w0)
+    t = 0.0
+    while t < T:
+        s.step(8)
+        t = s.get_time()[0]
+    a = s.get_state().reshape(wl.modes, 4, -1)[:, 0]
+    b = w0.reshape(wl.modes, 4, -1)[:, 0]
+    return float(np.mean(np.sqrt(np.sum((a - b) ** 2, axis=0))))
+
+
+@pytest.mark.parametrize("degree,meshes,floor", [(2, (24, 48), 2.7), (3, (16, 32), 3.3)])
+def test_isentropic_vortex_convergence_order(degree, meshes, floor):
+    """PAPER.md:444-470 (Fig. 5): the error of the steady vortex falls with the order p = n+1 of the scheme under mesh
+    refinement.  Run on the GPU to t = 1; the oracle gives 3.05 (degree 2, 24 -> 48 cells per axis) and 3.69 (degree 3,
+    16 -> 32: not yet asymptotic, the periodic box cuts the vortex tails at 1e-5), see tests/test_oracle_physics.py."""
+    e1, e2 = (_vortex_error(make_gpu, degree, N) for N in meshes)
+    order = np.log2(e1 / e2)
+    assert floor < order < degree + 1.6, (e1, e2, order)
+    _report("isentropic vortex degree %d: error %.3e (N = %d) -> %.3e (N = %d), order %.2f" % (
+        degree, e1, meshes[0], e2, meshes[1], order))

@@ -484,3 +484,22 @@ def test_eq23_separate_maxima_in_different_cells():
         wrong = 0.4 * o.h / (2 * (n + 1) * max(cs_cold + 3.0, cs_hot, cs_bg))
         assert abs(dt - right) < 1e-15
         assert abs(dt - wrong) > 0.2 * right
+
+
+def test_isentropic_vortex_convergence_order_of_the_oracle():
+    """PAPER.md:444-470 (Eq. 48-51, Fig. 5): the isentropic vortex is a steady solution, so the distance of the
+    solution at time T from the initial projection is the error of the scheme; under mesh refinement it falls with the
+    order p = n + 1.  Degree 2, 16 -> 32 cells per axis, T = 0.5."""
+    def err(N):
+        wl = wk.vortex(N, degree=2)
+        w0 = wk.initial_modes(wl)
+        o = orc.DGOracle(wl.dim, wl.ncell, wl.h, wl.order, wl.gamma, 0.0, 0.0, orc.Options(f_cfl=wl.f_cfl))
+        o.set_state(w0)
+        while o.t < 0.5:
+            assert o.step(1) == 0
+        a = o.get_state().reshape(wl.modes, 4, -1)[:, 0]
+        b = w0.reshape(wl.modes, 4, -1)[:, 0]
+        return float(np.mean(np.sqrt(np.sum((a - b) ** 2, axis=0))))
+
+    e1, e2 = err(16), err(32)
+    assert 2.6 < np.log2(e1 / e2) < 3.6, (e1, e2)

@@ -31,7 +31,7 @@ from paper_2208_11131_b200 import workloads as wk         # noqa: E402
 # dram__bytes_read.sum + dram__bytes_write.sum of one RK stage = one dg_face_kernel launch + one dg_stage2_kernel launch
 # (the middle RK3 stage, which reads u^n and u^(i-1)), from the newest committed ncu capture under profiles/, keyed by
 # (workload, degree).  A constant from that capture, not a live measurement; None where no capture exists.
-TRAFFIC_BYTES = {("cfg4", 3): {"face": 11.33e9, "stage": 21.45e9, "source": "profiles/r2b_cfg4.md"},
+TRAFFIC_BYTES = {("cfg4", 3): {"face": 11.33e9, "stage": 21.46e9, "source": "profiles/r3b_cfg4_ncu.md"},
                  ("cfg5", 7): {"face": 9.35e9, "stage": 18.78e9, "source": "profiles/r2b_cfg4.md"}}
 
 METRIC = "DG DoF-updates/sec (fp64, per RK stage)"
